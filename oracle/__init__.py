@@ -1,0 +1,196 @@
+"""CPU oracle (test infrastructure, not the product): ctypes view of oracle/lqcd_oracle.cpp.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It imports nothing from paper_2503_16994_b200 and shares no code with the CUDA path.
+All arrays are numpy complex128 / float64 in the canonical layouts of SURVEY.md 8(b):
+gauge [V,4,3,3], spinor [V,4,3], clover blocks [V,2,6,6], site n = x1 + L1*(x2 + L2*(x3 + L3*x4)).
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lqcd_oracle.cpp")
+_LIB = os.path.join(_HERE, "liblqcd_oracle.so")
+
+BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB = 0, 1, 2, 3
+
+
+def build(force=False):
+    """Compile the oracle with g++ -O2 -fopenmp (no fast-math: fp64 results must be plain IEEE)."""
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+        return _LIB
+    cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC]
+    subprocess.check_call(cmd)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.oracle_plaquette.restype = ctypes.c_double
+        _lib.oracle_cg.restype = ctypes.c_int
+        _lib.oracle_cg_eo.restype = ctypes.c_int
+        _lib.oracle_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _c(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    if shape is not None:
+        assert a.shape == tuple(shape), (a.shape, shape)
+    return a
+
+
+def _L(L):
+    return (ctypes.c_int * 4)(*[int(v) for v in L])
+
+
+def _d(v, n):
+    if v is None:
+        v = [0.0] * n
+    return (ctypes.c_double * n)(*[float(t) for t in v])
+
+
+def vol(L):
+    return int(L[0]) * int(L[1]) * int(L[2]) * int(L[3])
+
+
+def num_threads():
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n):
+    lib().oracle_set_num_threads(ctypes.c_int(int(n)))
+
+
+def gamma(mu):
+    """gamma_mu for mu = 0..3 (directions 1..4), gamma5 for mu = 4, as 4x4 complex (D2)."""
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().oracle_gamma(ctypes.c_int(mu), _p(out))
+    return out
+
+
+def sigma(mu, nu):
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().oracle_sigma(ctypes.c_int(mu), ctypes.c_int(nu), _p(out))
+    return out
+
+
+def plaquette(L, U):
+    U = _c(U, (vol(L), 4, 3, 3))
+    return float(lib().oracle_plaquette(_L(L), _p(U)))
+
+
+def fhat_site(L, U, x, mu, nu, bc=BC_PERIODIC, phiT=None):
+    U = _c(U, (vol(L), 4, 3, 3))
+    out = np.zeros((3, 3), dtype=np.complex128)
+    lib().oracle_fhat_site(_L(L), ctypes.c_int(bc), _d(phiT, 3), _p(U), _L(x), ctypes.c_int(mu),
+                           ctypes.c_int(nu), _p(out))
+    return out
+
+
+def clover_dense(L, U, kappa, csw, bc=BC_PERIODIC, phiT=None, ct=1.0):
+    U = _c(U, (vol(L), 4, 3, 3))
+    out = np.zeros((vol(L), 12, 12), dtype=np.complex128)
+    lib().oracle_clover_dense(_L(L), ctypes.c_int(bc), _d(phiT, 3), ctypes.c_double(kappa),
+                              ctypes.c_double(csw), ctypes.c_double(ct), _p(U), _p(out))
+    return out
+
+
+def clover_blocks(L, U, kappa, csw, bc=BC_PERIODIC, phiT=None, ct=1.0):
+    U = _c(U, (vol(L), 4, 3, 3))
+    out = np.zeros((vol(L), 2, 6, 6), dtype=np.complex128)
+    lib().oracle_clover_blocks(_L(L), ctypes.c_int(bc), _d(phiT, 3), ctypes.c_double(kappa),
+                               ctypes.c_double(csw), ctypes.c_double(ct), _p(U), _p(out))
+    return out
+
+
+def clover_inverse(L, Ablk):
+    Ablk = _c(Ablk, (vol(L), 2, 6, 6))
+    out = np.zeros_like(Ablk)
+    lib().oracle_clover_inverse(_L(L), _p(Ablk), _p(out))
+    return out
+
+
+def dw(L, U, psi, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, dagger=False):
+    U = _c(U, (vol(L), 4, 3, 3))
+    psi = _c(psi, (vol(L), 4, 3))
+    out = np.zeros_like(psi)
+    ap = None
+    if Ablk is not None:
+        Ablk = _c(Ablk, (vol(L), 2, 6, 6))
+        ap = _p(Ablk)
+    lib().oracle_dw(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(psi),
+                    _p(out), ctypes.c_int(1 if dagger else 0))
+    return out
+
+
+def hop(L, U, psi, bc=BC_PERIODIC, theta=None):
+    U = _c(U, (vol(L), 4, 3, 3))
+    psi = _c(psi, (vol(L), 4, 3))
+    out = np.zeros_like(psi)
+    lib().oracle_hop(_L(L), ctypes.c_int(bc), _d(theta, 4), _p(U), _p(psi), _p(out))
+    return out
+
+
+def dw_at_sites(L, U, psi, sites, kappa, csw, bc=BC_PERIODIC, theta=None, phiT=None, ct=1.0, dagger=False):
+    U = _c(U, (vol(L), 4, 3, 3))
+    psi = _c(psi, (vol(L), 4, 3))
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.zeros((len(sites), 4, 3), dtype=np.complex128)
+    lib().oracle_dw_at_sites(_L(L), ctypes.c_int(bc), _d(theta, 4), _d(phiT, 3), ctypes.c_double(kappa),
+                             ctypes.c_double(csw), ctypes.c_double(ct), _p(U), _p(psi),
+                             ctypes.c_int(1 if dagger else 0), ctypes.c_long(len(sites)), _p(sites), _p(out))
+    return out
+
+
+def dhat(L, U, psi, kappa, Ablk, Ainv, bc=BC_PERIODIC, theta=None, dagger=False):
+    U = _c(U, (vol(L), 4, 3, 3))
+    psi = _c(psi, (vol(L), 4, 3))
+    Ablk = _c(Ablk, (vol(L), 2, 6, 6))
+    Ainv = _c(Ainv, (vol(L), 2, 6, 6))
+    out = np.zeros_like(psi)
+    lib().oracle_dhat(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), _p(Ablk),
+                      _p(Ainv), _p(psi), _p(out), ctypes.c_int(1 if dagger else 0))
+    return out
+
+
+def cg(L, U, b, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter=10000):
+    """Returns (x, iters, rel_resid_normal, rel_resid_true); iters < 0 means maxiter was hit."""
+    U = _c(U, (vol(L), 4, 3, 3))
+    b = _c(b, (vol(L), 4, 3))
+    x = np.zeros_like(b)
+    ap = None
+    if Ablk is not None:
+        Ablk = _c(Ablk, (vol(L), 2, 6, 6))
+        ap = _p(Ablk)
+    rn, rt = ctypes.c_double(0), ctypes.c_double(0)
+    it = lib().oracle_cg(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(b),
+                         _p(x), ctypes.c_double(tol), ctypes.c_int(maxiter), ctypes.byref(rn),
+                         ctypes.byref(rt))
+    return x, int(it), rn.value, rt.value
+
+
+def cg_eo(L, U, b, kappa, Ablk, Ainv, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter=10000):
+    U = _c(U, (vol(L), 4, 3, 3))
+    b = _c(b, (vol(L), 4, 3))
+    Ablk = _c(Ablk, (vol(L), 2, 6, 6))
+    Ainv = _c(Ainv, (vol(L), 2, 6, 6))
+    x = np.zeros_like(b)
+    rn, rt = ctypes.c_double(0), ctypes.c_double(0)
+    it = lib().oracle_cg_eo(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), _p(Ablk),
+                            _p(Ainv), _p(b), _p(x), ctypes.c_double(tol), ctypes.c_int(maxiter),
+                            ctypes.byref(rn), ctypes.byref(rt))
+    return x, int(it), rn.value, rt.value
