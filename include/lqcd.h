@@ -1,0 +1,148 @@
+/* lqcd.h -- C-ABI of the B200-native clover Wilson-Dirac / CG library (liblqcd_b200.so).
+ *
+ * What is computed is fixed by DESIGN.md ("Definitions D1-D8", restating SURVEY.md 8(c)); the paper
+ * (arxiv 2503.16994, LatticeGPU.jl) names the operations and their arguments:
+ *   SpaceParm  : lattice extents with time last, boundary conditions          PAPER.md:41-60  (sec. 2.1)
+ *   DiracParam : m0 <-> kappa, csw, theta (boundary phases), cF = c~_t
+ *   Dw!, g5Dw!, DwdagDw!(pso,U,psi,...) : out-of-place operator application
+ *   Csw!(dws,U,gp,lp) : clover term stored in a workspace field, used by Dw
+ *   CG!, propagator!(psi,U,dpar,dws,lp,maxiter,tol,...) -> iteration count
+ *   GaugeParm phi : SF boundary links exp(i phi/L)
+ *
+ * Conventions
+ *  - Every call returns lqcd_status (0 = OK, negative = error); nothing throws or aborts;
+ *    lqcd_last_error() returns a thread-local message for the last failing call.
+ *  - All field pointers are DEVICE pointers owned by the caller (e.g. torch allocations), at least
+ *    lqcd_field_bytes() long and 16-byte aligned.  `stream` is a cudaStream_t cast to void* (NULL =
+ *    default stream).  Calls are asynchronous on `stream`, except lqcd_cg_solve / lqcd_propagator /
+ *    the *_host convenience calls, which synchronise before returning.
+ *  - Inputs are const and left bit-unchanged; outputs must not alias inputs (LQCD_EINVAL).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns LQCD_ECUDA.
+ *  - "canonical" (interchange) layout, always fp64 complex (re,im), site n = x1 + L1*(x2 + L2*(x3 + L3*x4)),
+ *    x4 = time:   gauge  [n][mu=0..3][row][col]   (18 reals per link, mu=3 is time)
+ *                 spinor [n][spin=0..3][colour=0..2]
+ *                 clover [n][chirality=0..1][6][6]  dense Hermitian blocks, row = 3*s + a
+ *  - "internal" layout: private, tile-blocked even-odd structure of arrays;
+ *    only this library reads or writes it.  A full internal field is [even half | odd half]; the
+ *    even-odd operator works on the even half (first lqcd_field_bytes/2 bytes of a spinor).
+ *  - gamma basis, sign and normalisation conventions: DESIGN.md D2-D6.  D = A - kappa*H,
+ *    kappa = 1/(2(m0+4)), D_paper = D/(2 kappa).
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LQCD_OK = 0,
+  LQCD_EINVAL = -1,      /* bad argument (odd extent, aliasing, NULL pointer, bad enum)            */
+  LQCD_ENOMEM = -2,
+  LQCD_ECUDA = -3,       /* CUDA runtime error or no device                                         */
+  LQCD_ENOTCONV = -4,    /* CG hit maxiter; x holds the last iterate                                */
+  LQCD_EBREAKDOWN = -5,  /* CG saw a NaN or a non-positive <p, D^+D p>                              */
+  LQCD_EUNSUPPORTED = -6
+} lqcd_status;
+
+typedef enum { LQCD_BC_PERIODIC = 0, LQCD_BC_OPEN = 1, LQCD_BC_SF_ORBI = 2, LQCD_BC_SF_AFWB = 3 } lqcd_bc;
+typedef enum { LQCD_F64 = 0, LQCD_F32 = 1 } lqcd_prec;
+typedef enum { LQCD_RECON_18 = 18, LQCD_RECON_12 = 12 } lqcd_recon;
+typedef enum { LQCD_FIELD_GAUGE = 0, LQCD_FIELD_SPINOR = 1, LQCD_FIELD_CLOVER = 2, LQCD_FIELD_WORKSPACE = 3 } lqcd_field_kind;
+
+/* Geometry (the paper's SpaceParm, plus the fermion phases of DiracParam, :119). */
+typedef struct {
+  int L[4];            /* extents, L[3] = time; all even and >= 2; >= 4 in time for open/SF */
+  lqcd_bc bc;          /* PAPER.md:53-58.  SF_ORBI and SF_AFWB are the same for the fermion path (R9)     */
+  double theta[4];     /* ANGLES: every link of direction mu carries exp(i*theta[mu]/L[mu]) (R6)          */
+  double phi0[3];      /* SF only, informational: phases of the x4=0 boundary links, which the caller     */
+                       /* stores in the gauge array itself (R8)                                          */
+  double phiT[3];      /* SF only: phases of the x4=T boundary links W'_k = exp(i*phiT/L_k) */
+  int device;          /* CUDA ordinal                                                                   */
+} lqcd_geom_desc;
+
+/* Dirac parameters: kappa = 1/(2(m0+4)); csw; ct = c~_t (paper's cF), 1 = absent. */
+typedef struct { double kappa, csw, ct; } lqcd_dirac;
+
+typedef struct lqcd_geom lqcd_geom;   /* opaque, library-owned */
+
+lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out);
+lqcd_status lqcd_geom_destroy(lqcd_geom* g);
+/* tile shape (4 ints), tiles per direction (4 ints) and L2 chunking (2 ints) chosen for this lattice */
+lqcd_status lqcd_geom_info(const lqcd_geom* g, int tile[4], int ntiles[4], int chunk[2]);
+
+/* Bytes of one internal field.  WORKSPACE: what lqcd_cg_solve / lqcd_propagator need (prec = LQCD_F64
+ * covers the mixed-precision solver too). */
+size_t lqcd_field_bytes(const lqcd_geom* g, lqcd_field_kind kind, lqcd_prec prec, lqcd_recon recon);
+
+/* canonical (fp64) <-> internal.  Import rounds once to `prec` (R14). */
+lqcd_status lqcd_gauge_import(const lqcd_geom* g, const void* canon, void* U, lqcd_prec prec, lqcd_recon recon, void* stream);
+lqcd_status lqcd_gauge_export(const lqcd_geom* g, const void* U, void* canon, lqcd_prec prec, lqcd_recon recon, void* stream);
+lqcd_status lqcd_spinor_import(const lqcd_geom* g, const void* canon, void* psi, lqcd_prec prec, void* stream);
+lqcd_status lqcd_spinor_export(const lqcd_geom* g, const void* psi, void* canon, lqcd_prec prec, void* stream);
+lqcd_status lqcd_clover_export(const lqcd_geom* g, const void* clover, void* canon, lqcd_prec prec, void* stream);
+/* internal fp64 spinor/clover/gauge -> internal fp32 (round to nearest), same geometry */
+lqcd_status lqcd_field_to_f32(const lqcd_geom* g, lqcd_field_kind kind, lqcd_recon recon, const void* src64, void* dst32, void* stream);
+
+/* Csw! (D4, D5): A(x) = 1 + kappa*csw*(i/2) sum sigma_{mu nu} F^_{mu nu}(x) as two packed 6x6
+ * Hermitian blocks per site; F^ = (Q - Q^+)/8 from the four plaquette leaves.  Always evaluated in fp64
+ * from fp64 links `U64` (R14) and stored in `out_prec`.  clover_inv (may be NULL) receives A^{-1}. */
+lqcd_status lqcd_clover_build(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, lqcd_recon recon,
+                              void* clover, void* clover_inv, lqcd_prec out_prec, void* stream);
+
+/* Dw! (D6): out = A in - kappa H in.  clover == NULL => A = 1 (csw term absent until Csw!
+ * has been called).  lqcd_dwdag_apply: out = gamma5 D gamma5 in. */
+lqcd_status lqcd_dw_apply(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* clover,
+                          const void* in, void* out, lqcd_prec prec, lqcd_recon recon, void* stream);
+lqcd_status lqcd_dwdag_apply(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* clover,
+                             const void* in, void* out, lqcd_prec prec, lqcd_recon recon, void* stream);
+/* Even-odd preconditioned operator (D8) on even-site half fields:
+ * out_e = A_ee in_e - kappa^2 H_eo A_oo^{-1} H_oe in_e (dagger: gamma5 . gamma5).  tmp: one spinor field. */
+lqcd_status lqcd_dw_eo_apply(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* clover,
+                             const void* clover_inv, const void* in_e, void* out_e, void* tmp, int dagger,
+                             lqcd_prec prec, lqcd_recon recon, void* stream);
+
+/* b = delta_{x,y} e_{spin,colour} in the internal layout (propagator! point-source method). */
+lqcd_status lqcd_point_source(const lqcd_geom* g, const int y[4], int spin, int colour, void* b, lqcd_prec prec, void* stream);
+
+/* CG! on the normal equations (algorithm and stopping rule: DESIGN.md R11):
+ *   solves D x = b via D^+D x = D^+ b from x0 = 0 until |r| <= tol*|D^+ b| (recursive residual).
+ *   eo != 0   : even-odd preconditioned (D8), needs clover and clover_inv.
+ *   mixed != 0: defect correction, fp32 inner CG to inner_tol, fp64 outer; needs the *32 fields. */
+typedef struct { double tol; int maxiter; int mixed; int eo; double inner_tol; int check_every; } lqcd_cg_parm;
+typedef struct { int iters; int outer; double rel_resid_normal; double rel_resid_true; double seconds; } lqcd_cg_info;
+typedef struct {
+  const void* U64; const void* clover64; const void* clover_inv64;   /* fp64 internal fields             */
+  const void* U32; const void* clover32; const void* clover_inv32;   /* fp32 copies (mixed only, else NULL) */
+} lqcd_cg_fields;
+lqcd_status lqcd_cg_solve(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b,
+                          void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
+                          lqcd_recon recon, void* stream);
+
+/* propagator! point-source method: for column = 3*spin + colour = 0..11 solve D x = delta_y e_column
+ * with lqcd_cg_solve's parameters.  `columns`: 12 consecutive internal fp64 spinor fields (caller-owned, out);
+ * infos[12] filled per column.  Stops at the first column that fails and returns its status. */
+lqcd_status lqcd_propagator(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4],
+                            void* columns, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info infos[12],
+                            lqcd_recon recon, void* stream);
+
+/* BLAS-1 used by the solver, exported for tests: |v|^2 and <u,v> over a full (or even-half) spinor. */
+lqcd_status lqcd_spinor_norm2(const lqcd_geom* g, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream);
+lqcd_status lqcd_spinor_dot(const lqcd_geom* g, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host /* re, im */, void* stream);
+
+/* End-to-end convenience over HOST buffers in the canonical layout (allocates device scratch, copies in,
+ * imports, builds the clover term if csw != 0, applies D or D^+, exports, copies back). */
+lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host,
+                               const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
+                               lqcd_recon recon);
+
+const char* lqcd_last_error(void);
+/* number of kernels launched by this library since load (for bench.py's gpu_launches) */
+long long lqcd_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

@@ -1,0 +1,619 @@
+// api.cu -- the C-ABI of include/lqcd.h: argument checks, geometry, solver drivers.  No compute here
+// beyond launching the kernels of dw.cu / clover.cu / layout.cu / blas.cu; there is no CPU fallback.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <atomic>
+#include <chrono>
+
+#include "cg.cuh"
+
+namespace lqcd {
+
+static thread_local char g_err[512] = "";
+static std::atomic<long long> g_launches(0);
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  set_error("%s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+void count_launch(int n) { g_launches += n; }
+
+static int ilog2(int v) {
+  int l = 0;
+  while ((1 << l) < v) l++;
+  return l;
+}
+
+// largest power of two <= cap that divides L
+static int pow2_divisor(int L, int cap) {
+  int b = 1;
+  while (b * 2 <= cap && L % (b * 2) == 0) b *= 2;
+  return b;
+}
+
+static bool parse_ints(const char* s, int* out, int n) {
+  if (!s) return false;
+  for (int i = 0; i < n; i++) {
+    char* end;
+    long v = strtol(s, &end, 10);
+    if (end == s) return false;
+    out[i] = (int)v;
+    s = end;
+    if (*s == ',' || *s == 'x') s++;
+  }
+  return true;
+}
+
+// Tile shape: 8x4x4x2 sites (TV = 128 per parity, 256 threads for the full operator) when the extents
+// allow it; smaller powers of two otherwise; a longer time extent of the tile when the spatial one is short.
+static void choose_tiling(Geom& g) {
+  int b[4];
+  b[0] = pow2_divisor(g.L[0], 8);
+  b[1] = pow2_divisor(g.L[1], 4);
+  b[2] = pow2_divisor(g.L[2], 4);
+  b[3] = 2;
+  int env[4];
+  if (parse_ints(getenv("LQCD_TILE"), env, 4)) {
+    bool ok = true;
+    for (int i = 0; i < 4; i++)
+      ok = ok && env[i] >= 2 && (env[i] & (env[i] - 1)) == 0 && g.L[i] % env[i] == 0;
+    if (ok && (env[0] / 2) * env[1] * env[2] * env[3] <= 128)
+      for (int i = 0; i < 4; i++) b[i] = env[i];
+  } else {
+    while ((b[0] / 2) * b[1] * b[2] * b[3] < 128 && g.L[3] % (b[3] * 2) == 0 && b[3] < 8) b[3] *= 2;
+  }
+  for (int i = 0; i < 4; i++) {
+    g.b[i] = b[i];
+    g.nt[i] = g.L[i] / b[i];
+  }
+  g.lb[0] = ilog2(b[0] / 2);
+  for (int i = 1; i < 4; i++) g.lb[i] = ilog2(b[i]);
+  g.TV = (b[0] / 2) * b[1] * b[2] * b[3];
+  g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
+  // L2 chunking: sweep time inside a chunk of (c1 x c2) tiles in (x2, x3) so that one time layer of the chunk
+  // (the reuse distance of a time-neighbour) stays well inside L2; cut as few faces as possible.
+  long budget = 32768;
+  if (getenv("LQCD_LAYER_SITES")) budget = atol(getenv("LQCD_LAYER_SITES"));
+  int best1 = 1, best2 = 1;
+  double best_cost = 1e30;
+  long best_sites = 0;
+  for (int c1 = 1; c1 <= g.nt[1]; c1++) {
+    if (g.nt[1] % c1) continue;
+    for (int c2 = 1; c2 <= g.nt[2]; c2++) {
+      if (g.nt[2] % c2) continue;
+      long sites = (long)g.L[0] * c1 * b[1] * c2 * b[2] * b[3];
+      if (sites > budget && !(c1 == 1 && c2 == 1)) continue;
+      double cost = (c1 < g.nt[1] ? 1.0 / (c1 * b[1]) : 0.0) + (c2 < g.nt[2] ? 1.0 / (c2 * b[2]) : 0.0);
+      if (cost < best_cost - 1e-12 || (fabs(cost - best_cost) <= 1e-12 && sites > best_sites)) {
+        best_cost = cost; best_sites = sites; best1 = c1; best2 = c2;
+      }
+    }
+  }
+  int ce[2];
+  if (parse_ints(getenv("LQCD_CHUNK"), ce, 2) && ce[0] >= 1 && ce[1] >= 1 && g.nt[1] % ce[0] == 0 && g.nt[2] % ce[1] == 0) {
+    best1 = ce[0]; best2 = ce[1];
+  }
+  g.c1 = best1;
+  g.c2 = best2;
+}
+
+static cudaStream_t as_stream(void* s) { return (cudaStream_t)s; }
+
+static size_t spinor_complex(const Geom& g) { return (size_t)2 * g.Vh * 12; }
+static size_t elem_bytes(lqcd_prec p) { return p == LQCD_F64 ? sizeof(double2) : sizeof(float2); }
+static size_t partial_len(const Geom& g) {
+  size_t n = (size_t)g.ntiles;
+  size_t r = (size_t)2 * reduce_blocks(spinor_complex(g));
+  return (n > r ? n : r) + 64;
+}
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static bool valid_prec(lqcd_prec p) { return p == LQCD_F64 || p == LQCD_F32; }
+static bool valid_recon(lqcd_recon r) { return r == LQCD_RECON_18 || r == LQCD_RECON_12; }
+
+// workspace carving
+struct Workspace {
+  char* base;
+  size_t off;
+  void* take(size_t bytes) {
+    void* p = base + off;
+    off += align256(bytes);
+    return p;
+  }
+};
+
+static const int WS_SPINORS64 = 8;   // r,p,t,tmp, b', b^, b-masked, + the source of lqcd_propagator
+static const int WS_SPINORS32 = 6;
+
+}  // namespace lqcd
+
+using namespace lqcd;
+
+#define REQUIRE(cond, ...)          \
+  do {                              \
+    if (!(cond)) {                  \
+      set_error(__VA_ARGS__);       \
+      return LQCD_EINVAL;           \
+    }                               \
+  } while (0)
+#define CUDA_TRY(e, what)                        \
+  do {                                           \
+    if (!cuda_ok((e), what)) return LQCD_ECUDA;  \
+  } while (0)
+
+extern "C" {
+
+const char* lqcd_last_error(void) { return g_err; }
+long long lqcd_launch_count(void) { return g_launches.load(); }
+
+lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
+  REQUIRE(desc && out, "lqcd_geom_create: NULL argument");
+  *out = nullptr;
+  REQUIRE(desc->bc >= LQCD_BC_PERIODIC && desc->bc <= LQCD_BC_SF_AFWB, "lqcd_geom_create: bad bc %d", (int)desc->bc);
+  for (int i = 0; i < 4; i++)
+    REQUIRE(desc->L[i] >= 2 && desc->L[i] % 2 == 0, "lqcd_geom_create: extent L[%d]=%d must be even and >= 2 (R13)", i, desc->L[i]);
+  if (desc->bc != LQCD_BC_PERIODIC) REQUIRE(desc->L[3] >= 4, "lqcd_geom_create: open/SF need L[3] >= 4");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    set_error("lqcd_geom_create: no CUDA device (this library has no CPU fallback)");
+    return LQCD_ECUDA;
+  }
+  REQUIRE(desc->device >= 0 && desc->device < ndev, "lqcd_geom_create: bad device %d", desc->device);
+  CUDA_TRY(cudaSetDevice(desc->device), "cudaSetDevice");
+  lqcd_geom* h = (lqcd_geom*)calloc(1, sizeof(lqcd_geom));
+  if (!h) { set_error("out of host memory"); return LQCD_ENOMEM; }
+  h->desc = *desc;
+  Geom& g = h->g;
+  for (int i = 0; i < 4; i++) g.L[i] = desc->L[i];
+  g.bc = (int)desc->bc;
+  g.Vh = (long long)g.L[0] * g.L[1] * g.L[2] * g.L[3] / 2;
+  choose_tiling(g);
+  h->has_theta = false;
+  for (int i = 0; i < 4; i++) {
+    double ang = desc->theta[i] / desc->L[i];
+    h->th_re[i] = cos(ang);
+    h->th_im[i] = sin(ang);
+    if (desc->theta[i] != 0.0) h->has_theta = true;
+  }
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device), "cudaGetDeviceProperties");
+  h->sm_count = prop.multiProcessorCount;
+  *out = h;
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_geom_destroy(lqcd_geom* g) {
+  if (g) free(g);
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_geom_info(const lqcd_geom* h, int tile[4], int ntiles[4], int chunk[2]) {
+  REQUIRE(h, "lqcd_geom_info: NULL geometry");
+  for (int i = 0; i < 4; i++) {
+    if (tile) tile[i] = h->g.b[i];
+    if (ntiles) ntiles[i] = h->g.nt[i];
+  }
+  if (chunk) { chunk[0] = h->g.c1; chunk[1] = h->g.c2; }
+  return LQCD_OK;
+}
+
+size_t lqcd_field_bytes(const lqcd_geom* h, lqcd_field_kind kind, lqcd_prec prec, lqcd_recon recon) {
+  if (!h) return 0;
+  const Geom& g = h->g;
+  size_t sites = (size_t)2 * g.Vh;
+  size_t eb = elem_bytes(prec);
+  switch (kind) {
+    case LQCD_FIELD_GAUGE: return sites * 4 * (recon == LQCD_RECON_12 ? 6 : 9) * eb;
+    case LQCD_FIELD_SPINOR: return sites * 12 * eb;
+    case LQCD_FIELD_CLOVER: return sites * 36 * eb;
+    case LQCD_FIELD_WORKSPACE: {
+      size_t sp64 = align256(sites * 12 * sizeof(double2)), sp32 = align256(sites * 12 * sizeof(float2));
+      return WS_SPINORS64 * sp64 + WS_SPINORS32 * sp32 + 2 * align256(partial_len(g) * sizeof(double)) + 4096;
+    }
+  }
+  return 0;
+}
+
+#define DISPATCH_PREC(prec, call_d, call_f) ((prec) == LQCD_F64 ? (call_d) : (call_f))
+
+lqcd_status lqcd_gauge_import(const lqcd_geom* h, const void* canon, void* U, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && canon && U && canon != U, "lqcd_gauge_import: NULL or aliased argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_gauge_import: bad precision / recon");
+  CUDA_TRY(DISPATCH_PREC(prec, gauge_import<double>(h->g, canon, U, recon, as_stream(stream)),
+                         gauge_import<float>(h->g, canon, U, recon, as_stream(stream))), "gauge_import");
+  return LQCD_OK;
+}
+lqcd_status lqcd_gauge_export(const lqcd_geom* h, const void* U, void* canon, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && canon && U && canon != U, "lqcd_gauge_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_gauge_export: bad precision / recon");
+  CUDA_TRY(DISPATCH_PREC(prec, gauge_export<double>(h->g, U, canon, recon, as_stream(stream)),
+                         gauge_export<float>(h->g, U, canon, recon, as_stream(stream))), "gauge_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_spinor_import(const lqcd_geom* h, const void* canon, void* psi, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && psi && canon != psi, "lqcd_spinor_import: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_spinor_import: bad precision");
+  CUDA_TRY(DISPATCH_PREC(prec, spinor_import<double>(h->g, canon, psi, as_stream(stream)),
+                         spinor_import<float>(h->g, canon, psi, as_stream(stream))), "spinor_import");
+  return LQCD_OK;
+}
+lqcd_status lqcd_spinor_export(const lqcd_geom* h, const void* psi, void* canon, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && psi && canon != psi, "lqcd_spinor_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_spinor_export: bad precision");
+  CUDA_TRY(DISPATCH_PREC(prec, spinor_export<double>(h->g, psi, canon, as_stream(stream)),
+                         spinor_export<float>(h->g, psi, canon, as_stream(stream))), "spinor_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_clover_export(const lqcd_geom* h, const void* clover, void* canon, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && clover && canon != clover, "lqcd_clover_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_clover_export: bad precision");
+  CUDA_TRY(DISPATCH_PREC(prec, clover_export<double>(h->g, clover, canon, as_stream(stream)),
+                         clover_export<float>(h->g, clover, canon, as_stream(stream))), "clover_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_field_to_f32(const lqcd_geom* h, lqcd_field_kind kind, lqcd_recon recon, const void* src64, void* dst32, void* stream) {
+  REQUIRE(h && src64 && dst32 && src64 != dst32, "lqcd_field_to_f32: NULL or aliased argument");
+  REQUIRE(kind == LQCD_FIELD_GAUGE || kind == LQCD_FIELD_SPINOR || kind == LQCD_FIELD_CLOVER, "lqcd_field_to_f32: bad kind");
+  size_t n = lqcd_field_bytes(h, kind, LQCD_F64, recon) / sizeof(double2);
+  CUDA_TRY(to_f32(src64, dst32, n, as_stream(stream)), "to_f32");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_clover_build(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, lqcd_recon recon, void* clover,
+                              void* clover_inv, lqcd_prec out_prec, void* stream) {
+  REQUIRE(h && d && U64 && clover, "lqcd_clover_build: NULL argument");
+  REQUIRE(valid_prec(out_prec) && valid_recon(recon), "lqcd_clover_build: bad precision / recon");
+  REQUIRE(clover != U64 && clover_inv != U64 && clover != clover_inv, "lqcd_clover_build: aliased buffers");
+  CloverParm cp;
+  cp.kappa = d->kappa; cp.csw = d->csw; cp.ct = d->ct;
+  for (int i = 0; i < 3; i++) cp.phiT[i] = h->desc.phiT[i];
+  CUDA_TRY(clover_build(h->g, cp, U64, (int)recon, clover, clover_inv, (int)out_prec, as_stream(stream)), "clover_build");
+  return LQCD_OK;
+}
+
+}  // extern "C"
+template <typename T>
+static cudaError_t dw_apply_t(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                              void* out, bool dagger, int recon, cudaStream_t s) {
+  Op<T> M;
+  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.recon = recon; M.eo = false;
+  return M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s);
+}
+
+extern "C" {
+static lqcd_status dw_common(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                             void* out, lqcd_prec prec, lqcd_recon recon, void* stream, bool dagger) {
+  REQUIRE(h && d && U && in && out, "lqcd_dw_apply: NULL argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply: bad precision / recon");
+  REQUIRE(out != in && out != U && out != clover, "lqcd_dw_apply: output aliases an input (PAPER.md:121: separate pso/psi)");
+  CUDA_TRY(DISPATCH_PREC(prec, dw_apply_t<double>(h, d, U, clover, in, out, dagger, (int)recon, as_stream(stream)),
+                         dw_apply_t<float>(h, d, U, clover, in, out, dagger, (int)recon, as_stream(stream))), "dw kernel");
+  return LQCD_OK;
+}
+lqcd_status lqcd_dw_apply(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                          void* out, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  return dw_common(h, d, U, clover, in, out, prec, recon, stream, false);
+}
+lqcd_status lqcd_dwdag_apply(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                             void* out, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  return dw_common(h, d, U, clover, in, out, prec, recon, stream, true);
+}
+
+}  // extern "C"
+template <typename T>
+static cudaError_t dw_eo_t(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* A, const void* Ainv,
+                           const void* in, void* out, void* tmp, bool dagger, int recon, cudaStream_t s) {
+  Op<T> M;
+  M.geom = h; M.U = U; M.A = A; M.Ainv = Ainv; M.tmp = tmp; M.kappa = d->kappa; M.recon = recon; M.eo = true;
+  return M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s);
+}
+extern "C" {
+lqcd_status lqcd_dw_eo_apply(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* clover_inv,
+                             const void* in_e, void* out_e, void* tmp, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && U && clover && clover_inv && in_e && out_e && tmp, "lqcd_dw_eo_apply: NULL argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_eo_apply: bad precision / recon");
+  REQUIRE(out_e != in_e && tmp != in_e && tmp != out_e, "lqcd_dw_eo_apply: aliased buffers");
+  CUDA_TRY(DISPATCH_PREC(prec, dw_eo_t<double>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream)),
+                         dw_eo_t<float>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream))),
+           "dw_eo kernel");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_point_source(const lqcd_geom* h, const int y[4], int spin, int colour, void* b, lqcd_prec prec, void* stream) {
+  REQUIRE(h && y && b, "lqcd_point_source: NULL argument");
+  REQUIRE(valid_prec(prec), "lqcd_point_source: bad precision");
+  REQUIRE(spin >= 0 && spin < 4 && colour >= 0 && colour < 3, "lqcd_point_source: bad spin/colour");
+  for (int i = 0; i < 4; i++) REQUIRE(y[i] >= 0 && y[i] < h->g.L[i], "lqcd_point_source: position outside the lattice");
+  CUDA_TRY(DISPATCH_PREC(prec, point_source<double>(h->g, y, spin, colour, b, as_stream(stream)),
+                         point_source<float>(h->g, y, spin, colour, b, as_stream(stream))), "point_source");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_spinor_norm2(const lqcd_geom* h, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream) {
+  REQUIRE(h && v && workspace && result_host, "lqcd_spinor_norm2: NULL argument");
+  REQUIRE(valid_prec(prec), "lqcd_spinor_norm2: bad precision");
+  size_t n = spinor_complex(h->g) / (half ? 2 : 1);
+  double* partial = (double*)workspace;
+  double* scratch = partial + partial_len(h->g) - 8;
+  CUDA_TRY(DISPATCH_PREC(prec, device_norm2<double>(v, n, partial, scratch, result_host, as_stream(stream)),
+                         device_norm2<float>(v, n, partial, scratch, result_host, as_stream(stream))), "norm2");
+  return LQCD_OK;
+}
+lqcd_status lqcd_spinor_dot(const lqcd_geom* h, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream) {
+  REQUIRE(h && u && v && workspace && result_host, "lqcd_spinor_dot: NULL argument");
+  REQUIRE(valid_prec(prec), "lqcd_spinor_dot: bad precision");
+  size_t n = spinor_complex(h->g) / (half ? 2 : 1);
+  double* partial = (double*)workspace;
+  double* scratch = partial + partial_len(h->g) - 8;
+  cudaStream_t s = as_stream(stream);
+  CUDA_TRY(DISPATCH_PREC(prec, dot_partial<double>(u, v, n, partial, s), dot_partial<float>(u, v, n, partial, s)), "dot");
+  CUDA_TRY(final_sum(partial, reduce_blocks(n), 2, scratch, s), "final_sum");
+  CUDA_TRY(cudaMemcpyAsync(result_host, scratch, 2 * sizeof(double), cudaMemcpyDeviceToHost, s), "memcpy");
+  CUDA_TRY(cudaStreamSynchronize(s), "sync");
+  return LQCD_OK;
+}
+
+}  // extern "C"
+// ---------------------------------------------------------------------------------------------------------
+// solver
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+
+struct SolveCtx {
+  const lqcd_geom* h;
+  const lqcd_dirac* d;
+  const lqcd_cg_fields* f;
+  const lqcd_cg_parm* parm;
+  int recon;
+  cudaStream_t s;
+  // workspace pieces
+  void* v64[WS_SPINORS64];
+  void* v32[WS_SPINORS32];
+  double* partial;
+  double* scratch;     // 8 doubles on the device
+  CgState* state;
+};
+
+template <typename T>
+Op<T> make_op(const SolveCtx& c, void* tmp) {
+  Op<T> M;
+  M.geom = c.h;
+  const bool f64 = sizeof(T) == 8;
+  M.U = f64 ? c.f->U64 : c.f->U32;
+  M.A = f64 ? c.f->clover64 : c.f->clover32;
+  M.Ainv = f64 ? c.f->clover_inv64 : c.f->clover_inv32;
+  M.tmp = tmp;
+  M.kappa = c.d->kappa;
+  M.recon = c.recon;
+  M.eo = c.parm->eo != 0;
+  return M;
+}
+
+#define CKS(e, what) do { if (!cuda_ok((e), what)) return LQCD_ECUDA; } while (0)
+
+// Solve M^+ M x = bp in fp64, plain or by defect correction with an fp32 inner CG.
+// Uses v64[0..2] (r,p,t), v64[3] (tmp for eo) and the fp32 vectors.  Returns iterations in *iters, outer count in *outer.
+lqcd_status solve_normal(const SolveCtx& c, const void* bp, void* x, int* iters, int* outer, double* rho0_out) {
+  Op<double> M = make_op<double>(c, c.v64[3]);
+  const size_t n = M.ncomplex();
+  CgVectors v;
+  v.r = c.v64[0]; v.p = c.v64[1]; v.t = c.v64[2]; v.partial = c.partial; v.state = c.state;
+  CgState hs;
+  const int check = c.parm->check_every > 0 ? c.parm->check_every : 16;
+  *outer = 0;
+  if (!c.parm->mixed) {
+    CKS(cg_normal<double>(M, bp, x, v, c.parm->tol, c.parm->maxiter, check, &hs, c.s), "cg_normal");
+    *iters = hs.iters;
+    *rho0_out = hs.rho0;
+    if (hs.breakdown) { set_error("lqcd_cg_solve: breakdown (NaN or <p,M^+M p> <= 0) at iteration %d", hs.iters); return LQCD_EBREAKDOWN; }
+    if (!hs.done) { set_error("lqcd_cg_solve: not converged after %d iterations", hs.iters); return LQCD_ENOTCONV; }
+    return LQCD_OK;
+  }
+  // mixed precision: r = bp - M^+M x (fp64); e = CG32(r) to inner_tol; x += e
+  Op<float> M32 = make_op<float>(c, c.v32[4]);
+  CgVectors w;
+  w.r = c.v32[1]; w.p = c.v32[2]; w.t = c.v32[3]; w.partial = c.partial; w.state = c.state;
+  void* r64 = c.v64[0];
+  void* t64 = c.v64[1];
+  void* q64 = c.v64[2];
+  double rho0 = 0, rho = 0;
+  CKS(cudaMemsetAsync(x, 0, n * sizeof(double2), c.s), "memset");
+  CKS(cudaMemcpyAsync(r64, bp, n * sizeof(double2), cudaMemcpyDeviceToDevice, c.s), "copy");
+  CKS(device_norm2<double>(r64, n, c.partial, c.scratch, &rho0, c.s), "norm2");
+  *rho0_out = rho0;
+  rho = rho0;
+  int total = 0;
+  const double inner_tol = c.parm->inner_tol > 0 ? c.parm->inner_tol : 1e-4;
+  for (;;) {
+    if (rho0 == 0.0 || rho <= c.parm->tol * c.parm->tol * rho0) break;
+    if (!(rho == rho)) { *iters = total; set_error("lqcd_cg_solve: NaN residual in mixed solve"); return LQCD_EBREAKDOWN; }
+    if (total >= c.parm->maxiter) { *iters = total; set_error("lqcd_cg_solve: not converged after %d inner iterations", total); return LQCD_ENOTCONV; }
+    CKS(to_f32(r64, c.v32[0], n, c.s), "to_f32");
+    // do not ask the inner solve for more than the outer one still needs
+    double need = c.parm->tol * sqrt(rho0 / rho) * 0.5;
+    double itol = inner_tol > need ? inner_tol : need;
+    CKS(cg_normal<float>(M32, c.v32[0], c.v32[5], w, itol, c.parm->maxiter - total, check, &hs, c.s), "cg_normal32");
+    total += hs.iters;
+    *outer += 1;
+    if (hs.breakdown) { *iters = total; set_error("lqcd_cg_solve: breakdown in the fp32 inner solve"); return LQCD_EBREAKDOWN; }
+    CKS(add_f32_to_f64(c.v32[5], x, n, c.s), "x += e");
+    CKS(M.apply(x, t64, false, EPI_STORE, nullptr, nullptr, nullptr, nullptr, c.s), "M x");
+    CKS(M.apply(t64, q64, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, c.s), "M^+ M x");
+    CKS(xmy<double>(bp, q64, r64, n, c.s), "r = bp - q");
+    CKS(device_norm2<double>(r64, n, c.partial, c.scratch, &rho, c.s), "norm2");
+  }
+  *iters = total;
+  return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b, void* x,
+                          void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && f && b && x && workspace && parm && info, "lqcd_cg_solve: NULL argument");
+  REQUIRE(valid_recon(recon), "lqcd_cg_solve: bad recon");
+  REQUIRE(f->U64, "lqcd_cg_solve: U64 is required");
+  REQUIRE(x != b, "lqcd_cg_solve: x aliases b");
+  REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve: bad tol / maxiter");
+  if (parm->eo) REQUIRE(f->clover64 && f->clover_inv64, "lqcd_cg_solve: eo needs clover64 and clover_inv64");
+  if (parm->mixed) {
+    REQUIRE(f->U32, "lqcd_cg_solve: mixed needs U32");
+    REQUIRE((f->clover64 == nullptr) == (f->clover32 == nullptr), "lqcd_cg_solve: mixed needs clover32 iff clover64");
+    if (parm->eo) REQUIRE(f->clover_inv32, "lqcd_cg_solve: mixed eo needs clover_inv32");
+  }
+  memset(info, 0, sizeof(*info));
+  auto t0 = std::chrono::steady_clock::now();
+  const Geom& g = h->g;
+  SolveCtx c;
+  c.h = h; c.d = d; c.f = f; c.parm = parm; c.recon = (int)recon; c.s = as_stream(stream);
+  Workspace ws{(char*)workspace, 0};
+  const size_t sites = (size_t)2 * g.Vh;
+  for (int i = 0; i < WS_SPINORS64; i++) c.v64[i] = ws.take(sites * 12 * sizeof(double2));
+  for (int i = 0; i < WS_SPINORS32; i++) c.v32[i] = ws.take(sites * 12 * sizeof(float2));
+  c.partial = (double*)ws.take(partial_len(g) * sizeof(double));
+  c.scratch = (double*)ws.take(64);
+  c.state = (CgState*)ws.take(sizeof(CgState));
+  const size_t nfull = spinor_complex(g);
+  cudaStream_t s = c.s;
+  lqcd_status st = LQCD_OK;
+  double rho0 = 0;
+  int iters = 0, outer = 0;
+
+  if (!parm->eo) {
+    Op<double> M = make_op<double>(c, nullptr);
+    void* bp = c.v64[4];
+    CKS(M.apply(b, bp, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^+ b");
+    st = solve_normal(c, bp, x, &iters, &outer, &rho0);
+    if (st != LQCD_OK && st != LQCD_ENOTCONV) { info->iters = iters; info->outer = outer; return st; }
+    // true residuals with fresh operator applications (R11)
+    void* t = c.v64[0];
+    void* q = c.v64[1];
+    double nb = 0, nr = 0, nq = 0;
+    CKS(M.apply(x, t, false, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D x");
+    CKS(xmy<double>(b, t, t, nfull, s), "b - Dx");
+    CKS(device_norm2<double>(b, nfull, c.partial, c.scratch, &nb, s), "norm2");
+    CKS(device_norm2<double>(t, nfull, c.partial, c.scratch, &nr, s), "norm2");
+    CKS(M.apply(t, q, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^+ (b - Dx)");
+    CKS(device_norm2<double>(q, nfull, c.partial, c.scratch, &nq, s), "norm2");
+    info->rel_resid_true = nb > 0 ? sqrt(nr / nb) : 0.0;
+    info->rel_resid_normal = rho0 > 0 ? sqrt(nq / rho0) : 0.0;
+  } else {
+    // D8: b^_e = b_e + kappa H_eo A_oo^{-1} b_o ; solve D^ x_e = b^_e ; x_o = A_oo^{-1} (b_o + kappa H_oe x_e)
+    Op<double> M = make_op<double>(c, c.v64[3]);
+    void* tmp = c.v64[3];   // full field scratch (odd half used)
+    void* bh = c.v64[4];    // b^_e   (even half)
+    void* bp = c.v64[5];    // D^^+ b^_e
+    void* bm = c.v64[6];    // b with the frozen slices zeroed
+    CKS(cudaMemcpyAsync(bm, b, nfull * sizeof(double2), cudaMemcpyDeviceToDevice, s), "copy b");
+    CKS(mask_frozen<double>(g, bm, s), "mask");
+    CKS(launch_diag<double>(g, f->clover_inv64, bm, tmp, 1, s), "A_oo^-1 b_o");
+    CKS(M.hop_xpay(tmp, bm, bh, -d->kappa, 0, s), "b_e + kappa H_eo .");
+    CKS(M.apply(bh, bp, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^^+ b^");
+    st = solve_normal(c, bp, x, &iters, &outer, &rho0);   // x even half
+    if (st != LQCD_OK && st != LQCD_ENOTCONV) { info->iters = iters; info->outer = outer; return st; }
+    // normal-equation residual of the preconditioned system
+    {
+      void* t = c.v64[0];
+      void* q = c.v64[1];
+      double nq = 0;
+      const size_t nh = nfull / 2;
+      CKS(M.apply(x, t, false, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^ x");
+      CKS(xmy<double>(bh, t, t, nh, s), "b^ - D^ x");
+      CKS(M.apply(t, q, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^^+ .");
+      CKS(device_norm2<double>(q, nh, c.partial, c.scratch, &nq, s), "norm2");
+      info->rel_resid_normal = rho0 > 0 ? sqrt(nq / rho0) : 0.0;
+    }
+    // odd part: tmp_o = b_o + kappa H_oe x_e ; x_o = A_oo^{-1} tmp_o   (x is a full field: even half solved above)
+    CKS(M.hop_xpay(x, bm, tmp, -d->kappa, 1, s), "b_o + kappa H_oe x_e");
+    CKS(launch_diag<double>(g, f->clover_inv64, tmp, x, 1, s), "A_oo^-1 .");
+    // true residual of the full system
+    {
+      Op<double> Mf = make_op<double>(c, nullptr);
+      Mf.eo = false;
+      void* t = c.v64[0];
+      double nb = 0, nr = 0;
+      CKS(Mf.apply(x, t, false, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D x");
+      CKS(xmy<double>(bm, t, t, nfull, s), "b - Dx");
+      CKS(device_norm2<double>(bm, nfull, c.partial, c.scratch, &nb, s), "norm2");
+      CKS(device_norm2<double>(t, nfull, c.partial, c.scratch, &nr, s), "norm2");
+      info->rel_resid_true = nb > 0 ? sqrt(nr / nb) : 0.0;
+    }
+  }
+  CKS(cudaStreamSynchronize(s), "sync");
+  info->iters = iters;
+  info->outer = outer;
+  info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  return st;
+}
+
+lqcd_status lqcd_propagator(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4], void* columns,
+                            void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info infos[12], lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && f && y && columns && workspace && parm && infos, "lqcd_propagator: NULL argument");
+  const size_t sbytes = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, LQCD_F64, recon);
+  // the source lives in the last fp64 workspace vector, which lqcd_cg_solve does not touch
+  void* b = (char*)workspace + (size_t)(WS_SPINORS64 - 1) * align256(sbytes);
+  for (int col = 0; col < 12; col++) {
+    lqcd_status st = lqcd_point_source(h, y, col / 3, col % 3, b, LQCD_F64, stream);
+    if (st != LQCD_OK) return st;
+    st = lqcd_cg_solve(h, d, f, b, (char*)columns + (size_t)col * sbytes, workspace, parm, &infos[col], recon, stream);
+    if (st != LQCD_OK) return st;
+  }
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host, const void* in_canon_host,
+                               void* out_canon_host, int dagger, lqcd_prec prec, lqcd_recon recon) {
+  REQUIRE(desc && d && U_canon_host && in_canon_host && out_canon_host, "lqcd_dw_apply_host: NULL argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply_host: bad precision / recon");
+  lqcd_geom* h = nullptr;
+  lqcd_status st = lqcd_geom_create(desc, &h);
+  if (st != LQCD_OK) return st;
+  const size_t V = (size_t)2 * h->g.Vh;
+  const size_t gc = V * 36 * sizeof(double2), sc = V * 12 * sizeof(double2);
+  void *dUc = nullptr, *dSc = nullptr, *dU64 = nullptr, *dU = nullptr, *dA = nullptr, *dIn = nullptr, *dOut = nullptr;
+  auto cleanup = [&]() {
+    cudaFree(dUc); cudaFree(dSc); cudaFree(dU64); if (dU != dU64) cudaFree(dU); cudaFree(dA); cudaFree(dIn); cudaFree(dOut);
+    lqcd_geom_destroy(h);
+  };
+#define HTRY(e, what) do { if (!cuda_ok((e), what)) { cleanup(); return LQCD_ECUDA; } } while (0)
+#define LTRY(e) do { lqcd_status _s = (e); if (_s != LQCD_OK) { cleanup(); return _s; } } while (0)
+  HTRY(cudaMalloc(&dUc, gc), "cudaMalloc");
+  HTRY(cudaMalloc(&dSc, sc), "cudaMalloc");
+  HTRY(cudaMalloc(&dU64, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F64, recon)), "cudaMalloc");
+  HTRY(cudaMalloc(&dIn, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
+  HTRY(cudaMalloc(&dOut, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
+  HTRY(cudaMemcpy(dUc, U_canon_host, gc, cudaMemcpyHostToDevice), "H2D gauge");
+  HTRY(cudaMemcpy(dSc, in_canon_host, sc, cudaMemcpyHostToDevice), "H2D spinor");
+  LTRY(lqcd_gauge_import(h, dUc, dU64, LQCD_F64, recon, nullptr));
+  if (d->csw != 0.0 || (desc->bc != LQCD_BC_PERIODIC && d->ct != 1.0)) {
+    HTRY(cudaMalloc(&dA, lqcd_field_bytes(h, LQCD_FIELD_CLOVER, prec, recon)), "cudaMalloc");
+    LTRY(lqcd_clover_build(h, d, dU64, recon, dA, nullptr, prec, nullptr));
+  }
+  if (prec == LQCD_F64) dU = dU64;
+  else {
+    HTRY(cudaMalloc(&dU, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F32, recon)), "cudaMalloc");
+    LTRY(lqcd_gauge_import(h, dUc, dU, LQCD_F32, recon, nullptr));
+  }
+  LTRY(lqcd_spinor_import(h, dSc, dIn, prec, nullptr));
+  LTRY(dw_common(h, d, dU, dA, dIn, dOut, prec, recon, nullptr, dagger != 0));
+  LTRY(lqcd_spinor_export(h, dOut, dSc, prec, nullptr));
+  HTRY(cudaMemcpy(out_canon_host, dSc, sc, cudaMemcpyDeviceToHost), "D2H spinor");
+  cleanup();
+#undef HTRY
+#undef LTRY
+  return LQCD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,250 @@
+// blas.cu -- BLAS-1 and reductions of the CG driver that are not fused into the stencil
+// (SURVEY.md 8(a) row a6): warp-shuffle trees, one partial per CTA, fixed-order final pass in a single
+// CTA (bit-reproducible run to run); fp64 accumulation in both precisions.  CG scalars stay on the device.
+#include "kernels.cuh"
+
+namespace lqcd {
+
+template <typename T> using T2 = typename vec2<T>::type;
+
+static const int RB_THREADS = 256;
+int reduce_blocks(size_t ncomplex) {
+  size_t b = (ncomplex + (size_t)RB_THREADS * 8 - 1) / ((size_t)RB_THREADS * 8);
+  if (b < 1) b = 1;
+  if (b > 148 * 8) b = 148 * 8;
+  return (int)b;
+}
+
+__device__ __forceinline__ double block_sum(double v, double* s_red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double s = 0;
+  if (threadIdx.x == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    for (int w = 0; w < nw; w++) s += s_red[w];
+  }
+  return s;  // valid in thread 0
+}
+
+template <typename T>
+__global__ void norm2_kernel(const T2<T>* __restrict__ v, size_t n, double* partial) {
+  __shared__ double s_red[32];
+  double acc = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> a = v[i];
+    acc += (double)a.x * (double)a.x + (double)a.y * (double)a.y;
+  }
+  double s = block_sum(acc, s_red);
+  if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+template <typename T>
+__global__ void dot_kernel(const T2<T>* __restrict__ u, const T2<T>* __restrict__ v, size_t n, double* partial) {
+  __shared__ double s_red[32];
+  double re = 0, im = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> a = u[i], b = v[i];  // conj(a) * b
+    re += (double)a.x * (double)b.x + (double)a.y * (double)b.y;
+    im += (double)a.x * (double)b.y - (double)a.y * (double)b.x;
+  }
+  double s = block_sum(re, s_red);
+  if (threadIdx.x == 0) partial[blockIdx.x] = s;
+  s = block_sum(im, s_red);
+  if (threadIdx.x == 0) partial[gridDim.x + blockIdx.x] = s;
+}
+
+// fixed-order sum of partial[0..n): thread t adds elements t, t+256, ... then a fixed tree
+__device__ double ordered_sum(const double* partial, int n, double* s_red) {
+  double acc = 0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) acc += partial[i];
+  return block_sum(acc, s_red);
+}
+
+__global__ void final_sum_kernel(const double* partial, int n, int nvals, double* result) {
+  __shared__ double s_red[32];
+  for (int k = 0; k < nvals; k++) {
+    double s = ordered_sum(partial + (size_t)k * n, n, s_red);
+    if (threadIdx.x == 0) result[k] = s;
+  }
+}
+
+__global__ void cg_init_kernel(CgState* st, const double* partial, int n, double tol) {
+  __shared__ double s_red[32];
+  double s = ordered_sum(partial, n, s_red);
+  if (threadIdx.x == 0) {
+    st->rho = s; st->rho0 = s; st->alpha = 0; st->beta = 0; st->tt = 0; st->rho_new = s;
+    st->tol2 = tol * tol;
+    st->iters = 0; st->breakdown = 0;
+    st->done = (s == 0.0) ? 1 : 0;
+    if (!(s == s)) { st->done = 1; st->breakdown = 1; }
+  }
+}
+
+// after t = M p:  alpha = rho / |t|^2
+__global__ void cg_alpha_kernel(CgState* st, const double* partial, int n) {
+  __shared__ double s_red[32];
+  if (st->done == 2) { if (threadIdx.x == 0) st->done = 1; return; }
+  if (st->done) return;
+  double s = ordered_sum(partial, n, s_red);
+  if (threadIdx.x == 0) {
+    st->tt = s;
+    if (!(s > 0.0)) { st->breakdown = 1; st->done = 1; st->alpha = 0; }
+    else st->alpha = st->rho / s;
+  }
+}
+
+// after r -= alpha M^+ t:  rho' = |r|^2, convergence test, beta = rho'/rho
+__global__ void cg_beta_kernel(CgState* st, const double* partial, int n) {
+  __shared__ double s_red[32];
+  if (st->done) return;
+  double s = ordered_sum(partial, n, s_red);
+  if (threadIdx.x == 0) {
+    st->rho_new = s;
+    st->iters += 1;
+    if (!(s == s)) { st->breakdown = 1; st->done = 2; st->alpha = 0; }
+    else if (s <= st->tol2 * st->rho0) st->done = 2;  // x += alpha p still pending
+    st->beta = s / st->rho;
+    st->rho = s;
+  }
+}
+
+template <typename T>
+__global__ void cg_update_xp_kernel(const CgState* st, T2<T>* x, T2<T>* p, const T2<T>* __restrict__ r, size_t n) {
+  const int done = st->done;
+  if (done == 1) return;
+  const T al = (T)st->alpha, be = (T)st->beta;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> xv = x[i], pv = p[i];
+    xv.x = fma(al, pv.x, xv.x);
+    xv.y = fma(al, pv.y, xv.y);
+    x[i] = xv;
+    if (done == 0) {
+      T2<T> rv = r[i];
+      pv.x = fma(be, pv.x, rv.x);
+      pv.y = fma(be, pv.y, rv.y);
+      p[i] = pv;
+    }
+  }
+}
+
+template <typename T>
+__global__ void axpy_kernel(T a, const T2<T>* __restrict__ x, T2<T>* y, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> xv = x[i], yv = y[i];
+    yv.x = fma(a, xv.x, yv.x);
+    yv.y = fma(a, xv.y, yv.y);
+    y[i] = yv;
+  }
+}
+template <typename T>
+__global__ void xmy_kernel(const T2<T>* __restrict__ x, const T2<T>* __restrict__ y, T2<T>* z, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> xv = x[i], yv = y[i];
+    xv.x -= yv.x; xv.y -= yv.y;
+    z[i] = xv;
+  }
+}
+__global__ void add32_kernel(const float2* __restrict__ e, double2* x, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    float2 ev = e[i];
+    double2 xv = x[i];
+    xv.x += (double)ev.x; xv.y += (double)ev.y;
+    x[i] = xv;
+  }
+}
+
+template <typename T>
+__global__ void mask_frozen_kernel(const Geom g, T2<T>* psi) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= 2 * g.Vh) return;
+  int p = (int)(idx / g.Vh);
+  long long rem = idx - (long long)p * g.Vh;
+  int tile = (int)(rem / g.TV);
+  int j = (int)(rem - (long long)tile * g.TV);
+  int Tc[4], l[4];
+  tile_coords(g, tile, Tc);
+  local_coords(g, j, p, l);
+  if (!frozen_slice(g, Tc[3] * g.b[3] + l[3])) return;
+  T2<T> z; z.x = 0; z.y = 0;
+  for (int c = 0; c < 12; c++) psi[field_offset(g, 12, p, tile, c, j)] = z;
+}
+
+static unsigned ew_blocks(size_t n) {
+  size_t b = (n + 1023) / 1024;
+  if (b < 1) b = 1;
+  if (b > 148 * 16) b = 148 * 16;
+  return (unsigned)b;
+}
+
+template <typename T> cudaError_t norm2_partial(const void* v, size_t n, double* partial, cudaStream_t s) {
+  norm2_kernel<T><<<reduce_blocks(n), RB_THREADS, 0, s>>>((const T2<T>*)v, n, partial);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t dot_partial(const void* u, const void* v, size_t n, double* partial, cudaStream_t s) {
+  dot_kernel<T><<<reduce_blocks(n), RB_THREADS, 0, s>>>((const T2<T>*)u, (const T2<T>*)v, n, partial);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t final_sum(const double* partial, int n, int nvals, double* result, cudaStream_t s) {
+  final_sum_kernel<<<1, 256, 0, s>>>(partial, n, nvals, result);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t cg_init_state(CgState* st, const double* partial, int n, double tol, cudaStream_t s) {
+  cg_init_kernel<<<1, 256, 0, s>>>(st, partial, n, tol);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t cg_reduce_alpha(CgState* st, const double* partial, int n, cudaStream_t s) {
+  cg_alpha_kernel<<<1, 256, 0, s>>>(st, partial, n);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t cg_reduce_beta(CgState* st, const double* partial, int n, cudaStream_t s) {
+  cg_beta_kernel<<<1, 256, 0, s>>>(st, partial, n);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void* p, const void* r, size_t n, cudaStream_t s) {
+  cg_update_xp_kernel<T><<<ew_blocks(n), 256, 0, s>>>(st, (T2<T>*)x, (T2<T>*)p, (const T2<T>*)r, n);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t axpy(double a, const void* x, void* y, size_t n, cudaStream_t s) {
+  axpy_kernel<T><<<ew_blocks(n), 256, 0, s>>>((T)a, (const T2<T>*)x, (T2<T>*)y, n);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t xmy(const void* x, const void* y, void* z, size_t n, cudaStream_t s) {
+  xmy_kernel<T><<<ew_blocks(n), 256, 0, s>>>((const T2<T>*)x, (const T2<T>*)y, (T2<T>*)z, n);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t add_f32_to_f64(const void* e32, void* x64, size_t n, cudaStream_t s) {
+  add32_kernel<<<ew_blocks(n), 256, 0, s>>>((const float2*)e32, (double2*)x64, n);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t mask_frozen(const Geom& g, void* psi, cudaStream_t s) {
+  if (g.bc == LQCD_BC_PERIODIC) return cudaSuccess;
+  mask_frozen_kernel<T><<<(unsigned)((2 * g.Vh + 255) / 256), 256, 0, s>>>(g, (T2<T>*)psi);
+  count_launch();
+  return cudaGetLastError();
+}
+
+#define INST(T)                                                                                     \
+  template cudaError_t norm2_partial<T>(const void*, size_t, double*, cudaStream_t);                \
+  template cudaError_t dot_partial<T>(const void*, const void*, size_t, double*, cudaStream_t);     \
+  template cudaError_t cg_update_xp<T>(const CgState*, void*, void*, const void*, size_t, cudaStream_t); \
+  template cudaError_t axpy<T>(double, const void*, void*, size_t, cudaStream_t);                   \
+  template cudaError_t xmy<T>(const void*, const void*, void*, size_t, cudaStream_t);               \
+  template cudaError_t mask_frozen<T>(const Geom&, void*, cudaStream_t);
+INST(double)
+INST(float)
+#undef INST
+
+}  // namespace lqcd

@@ -1,0 +1,125 @@
+// cg.cu -- CG! on the normal equations and the solves built on it (algorithm
+// and stopping rule: SURVEY.md 8(c) "Algorithm CG", R11; even-odd: D8; mixed precision: defect correction).
+//
+// One CG iteration is three big kernels:  t = M p with |t|^2 fused (EPI_STORE_NORM);  r -= alpha M^+ t with
+// |r|^2 fused, M^+ t never written (EPI_AXPY_NORM);  x += alpha p, p = r + beta p.  Two single-CTA kernels
+// turn the per-CTA partial sums into alpha, beta and the convergence flag on the device; the host reads
+// the 80-byte state back only every `check_every` iterations, and all kernels become no-ops once the flag
+// is set, so the iteration count is exact.
+#include <math.h>
+#include <string.h>
+
+#include "cg.cuh"
+
+namespace lqcd {
+
+template <typename T> using T2 = typename vec2<T>::type;
+
+#define CK(e) do { cudaError_t _e = (e); if (_e != cudaSuccess) return _e; } while (0)
+
+template <typename T>
+cudaError_t Op<T>::apply(const void* in, void* out, bool dagger, int epi, void* r, const double* alpha, double* partial,
+                         const int* skip, cudaStream_t s) const {
+  DwArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.U = (const T2<T>*)U;
+  a.r = (T2<T>*)r;
+  a.alpha = alpha;
+  a.partial = partial;
+  a.skip = skip;
+  a.has_theta = geom->has_theta;
+  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  a.dagger = dagger ? 1 : 0;
+  if (!eo) {
+    a.A = (const T2<T>*)A;
+    a.in = (const T2<T>*)in;
+    a.self = (const T2<T>*)in;
+    a.out = (T2<T>*)out;
+    a.k = (T)kappa;
+    a.parity = -1;
+    a.epi = epi;
+    return launch_dw<T>(geom->g, a, recon, A ? DIAG_PRE : DIAG_ONE, s);
+  }
+  // D^ = A_ee - kappa^2 H_eo A_oo^{-1} H_oe  (D8): tmp_o = A_oo^{-1} H_oe in_e ; out_e = A_ee in_e - kappa^2 H_eo tmp_o
+  a.A = (const T2<T>*)Ainv;
+  a.in = (const T2<T>*)in;
+  a.self = (const T2<T>*)in;
+  a.out = (T2<T>*)tmp;
+  a.k = (T)0;
+  a.parity = 1;
+  a.epi = EPI_STORE;
+  CK(launch_dw<T>(geom->g, a, recon, DIAG_POST, s));
+  a.A = (const T2<T>*)A;
+  a.in = (const T2<T>*)tmp;
+  a.self = (const T2<T>*)in;
+  a.out = (T2<T>*)out;
+  a.k = (T)(kappa * kappa);
+  a.parity = 0;
+  a.epi = epi;
+  return launch_dw<T>(geom->g, a, recon, DIAG_PRE, s);
+}
+
+// out(parity) = self - k * H in   (no clover), used by the even-odd source preparation / reconstruction
+template <typename T>
+cudaError_t Op<T>::hop_xpay(const void* in, const void* self, void* out, double k, int parity, cudaStream_t s) const {
+  DwArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.U = (const T2<T>*)U;
+  a.in = (const T2<T>*)in;
+  a.self = (const T2<T>*)self;
+  a.out = (T2<T>*)out;
+  a.k = (T)k;
+  a.has_theta = geom->has_theta;
+  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  a.parity = parity;
+  a.epi = EPI_STORE;
+  return launch_dw<T>(geom->g, a, recon, DIAG_ONE, s);
+}
+
+template <typename T>
+cudaError_t cg_normal(const Op<T>& M, const void* bprime, void* x, const CgVectors& v, double tol, int maxiter,
+                      int check_every, CgState* host_state, cudaStream_t s) {
+  const size_t n = M.ncomplex();
+  const size_t bytes = n * sizeof(T2<T>);
+  const int nt = M.geom->g.ntiles;
+  CK(cudaMemsetAsync(x, 0, bytes, s));
+  CK(cudaMemcpyAsync(v.r, bprime, bytes, cudaMemcpyDeviceToDevice, s));
+  CK(cudaMemcpyAsync(v.p, bprime, bytes, cudaMemcpyDeviceToDevice, s));
+  CK(norm2_partial<T>(v.r, n, v.partial, s));
+  CK(cg_init_state(v.state, v.partial, reduce_blocks(n), tol, s));
+  if (check_every < 1) check_every = 1;
+  int launched = 0;
+  for (;;) {
+    CK(cudaMemcpyAsync(host_state, v.state, sizeof(CgState), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (host_state->done || launched >= maxiter) break;
+    int batch = check_every;
+    if (launched + batch > maxiter) batch = maxiter - launched;
+    for (int it = 0; it < batch; it++) {
+      CK(M.apply(v.p, v.t, false, EPI_STORE_NORM, nullptr, nullptr, v.partial, &v.state->done, s));
+      CK(cg_reduce_alpha(v.state, v.partial, nt, s));
+      CK(M.apply(v.t, nullptr, true, EPI_AXPY_NORM, v.r, &v.state->alpha, v.partial, &v.state->done, s));
+      CK(cg_reduce_beta(v.state, v.partial, nt, s));
+      CK(cg_update_xp<T>(v.state, x, v.p, v.r, n, s));
+    }
+    launched += batch;
+  }
+  return cudaSuccess;
+}
+
+template <typename T>
+cudaError_t device_norm2(const void* vec, size_t n, double* partial, double* scratch_dev, double* host, cudaStream_t s) {
+  CK(norm2_partial<T>(vec, n, partial, s));
+  CK(final_sum(partial, reduce_blocks(n), 1, scratch_dev, s));
+  CK(cudaMemcpyAsync(host, scratch_dev, sizeof(double), cudaMemcpyDeviceToHost, s));
+  return cudaStreamSynchronize(s);
+}
+
+template struct Op<double>;
+template struct Op<float>;
+template cudaError_t cg_normal<double>(const Op<double>&, const void*, void*, const CgVectors&, double, int, int, CgState*, cudaStream_t);
+template cudaError_t cg_normal<float>(const Op<float>&, const void*, void*, const CgVectors&, double, int, int, CgState*, cudaStream_t);
+template cudaError_t device_norm2<double>(const void*, size_t, double*, double*, double*, cudaStream_t);
+template cudaError_t device_norm2<float>(const void*, size_t, double*, double*, double*, cudaStream_t);
+
+}  // namespace lqcd

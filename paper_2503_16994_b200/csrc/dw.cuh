@@ -1,0 +1,35 @@
+// dw.cuh -- arguments of the stencil kernel (dw.cu) and of the BLAS-1 / reduction kernels (blas.cu).
+#pragma once
+#include "lqcd_internal.cuh"
+
+namespace lqcd {
+
+enum { DIAG_ONE = 0, DIAG_PRE = 1, DIAG_POST = 2 };
+enum { EPI_STORE = 0, EPI_STORE_NORM = 1, EPI_AXPY_NORM = 2 };
+
+template <typename T>
+struct DwArgs {
+  const typename vec2<T>::type* U;     // internal gauge field
+  const typename vec2<T>::type* A;     // packed clover blocks (DIAG_PRE: A, DIAG_POST: A^{-1}); unused for DIAG_ONE
+  const typename vec2<T>::type* in;    // field whose neighbours are hopped (base of a full field)
+  const typename vec2<T>::type* self;  // field supplying the site-diagonal term (base of a full field)
+  typename vec2<T>::type* out;         // base of a full field (only the output parity is written)
+  typename vec2<T>::type* r;           // EPI_AXPY_NORM: r -= alpha * result
+  const double* alpha;                 // device scalar
+  double* partial;                     // one partial sum per CTA
+  const int* skip;                     // device flag: if non-NULL and *skip != 0 the kernel does nothing
+  T k;                                 // kappa (or kappa^2 for the even-odd operator)
+  cx<T> theta[4];
+  int has_theta;
+  int dagger;
+  int parity;                          // -1: both parities; 0/1: only this output parity
+  int epi;
+};
+
+template <typename T>
+cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cudaStream_t s);
+// out(x) = B(x) in(x) on sites of `parity` (-1: all), zero on frozen slices; B = packed 6x6 blocks
+template <typename T>
+cudaError_t launch_diag(const Geom& g, const void* B, const void* in, void* out, int parity, cudaStream_t s);
+
+}  // namespace lqcd

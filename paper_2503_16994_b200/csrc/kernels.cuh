@@ -1,0 +1,49 @@
+// kernels.cuh -- host-callable launchers of layout.cu, clover.cu and blas.cu.
+#pragma once
+#include "dw.cuh"
+
+namespace lqcd {
+
+// layout.cu
+template <typename T> cudaError_t gauge_import(const Geom& g, const void* canon, void* U, int recon, cudaStream_t s);
+template <typename T> cudaError_t gauge_export(const Geom& g, const void* U, void* canon, int recon, cudaStream_t s);
+template <typename T> cudaError_t spinor_import(const Geom& g, const void* canon, void* psi, cudaStream_t s);
+template <typename T> cudaError_t spinor_export(const Geom& g, const void* psi, void* canon, cudaStream_t s);
+template <typename T> cudaError_t clover_export(const Geom& g, const void* A, void* canon, cudaStream_t s);
+template <typename T> cudaError_t point_source(const Geom& g, const int y[4], int spin, int colour, void* b, cudaStream_t s);
+cudaError_t to_f32(const void* src, void* dst, size_t ncomplex, cudaStream_t s);
+
+// clover.cu
+struct CloverParm {
+  double kappa, csw, ct;
+  double phiT[3];
+};
+cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, int recon, void* clover, void* clover_inv,
+                         int out_prec, cudaStream_t s);
+
+// blas.cu -- CG scalars live on the device
+struct CgState {
+  double rho, rho0, alpha, beta, tt, rho_new, tol2;
+  int done;       // 0 running, 2 converged this iteration (x update pending), 1 finished
+  int iters;
+  int breakdown;
+  int pad;
+};
+int reduce_blocks(size_t ncomplex);  // grid size used by the norm/dot kernels (partial buffer length)
+template <typename T> cudaError_t norm2_partial(const void* v, size_t ncomplex, double* partial, cudaStream_t s);
+template <typename T> cudaError_t dot_partial(const void* u, const void* v, size_t ncomplex, double* partial, cudaStream_t s);
+cudaError_t final_sum(const double* partial, int n, int nvals, double* result, cudaStream_t s);
+// CG bookkeeping kernels (single CTA; partial sums reduced in fixed order)
+cudaError_t cg_init_state(CgState* st, const double* partial, int n, double tol, cudaStream_t s);
+cudaError_t cg_reduce_alpha(CgState* st, const double* partial, int n, cudaStream_t s);
+cudaError_t cg_reduce_beta(CgState* st, const double* partial, int n, cudaStream_t s);
+// x += alpha p ; p = r + beta p   (skips according to st->done)
+template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void* p, const void* r, size_t ncomplex, cudaStream_t s);
+// y = a*x + y  /  y = x + a*y  / copy / zero with host scalar a
+template <typename T> cudaError_t axpy(double a, const void* x, void* y, size_t ncomplex, cudaStream_t s);
+template <typename T> cudaError_t xmy(const void* x, const void* y, void* z, size_t ncomplex, cudaStream_t s);  // z = x - y
+cudaError_t add_f32_to_f64(const void* e32, void* x64, size_t ncomplex, cudaStream_t s);                          // x += e
+// zero the frozen time slices of a spinor (D7: the solve lives on the interior)
+template <typename T> cudaError_t mask_frozen(const Geom& g, void* psi, cudaStream_t s);
+
+}  // namespace lqcd
