@@ -1,0 +1,545 @@
+#!/usr/bin/env python
+"""bench.py -- Dw throughput of the clover Wilson-Dirac hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+One STEP is one application of the normal operator Dw^+ Dw (the paper's DwdagDw!; the body of
+every CG iteration): one lqcd_dw_apply followed by one lqcd_dwdag_apply on a fixed
+Gaussian spinor, on the 48^3 x 96 periodic lattice of BASELINE.json configs[4] (the configuration the
+north_star's >= 70 %-of-HBM-peak target is quoted on; configs[1], 16^3 x 32, is L2-resident and therefore
+not an HBM-roofline point).  metric = Dw GFLOP/s under the stated flop model (1872 flop/site/application).
+Inputs exceed L2 (16.3 GB compulsory traffic per application vs 126 MB), so no L2 flush is needed.
+
+The JSON line also carries: `roofline` (the stencil kernel against the measured HBM copy bandwidth of
+MEASURED_PEAKS.json, compulsory-bytes model of DESIGN.md), `e2e` (the same metric through the host-buffer
+C-ABI call lqcd_dw_apply_host, copies inside the timed region), `cpu_baseline` (the fp64 oracle timed on
+this box's host cores on a bounded sample) and `rows` (the other hot-path rows of SURVEY.md 8(a), each
+measured once in the same run on rank 0 at N=1).
+
+Multi-GPU: the path does not exchange data between GPUs ("replicas only"):
+each rank runs an independent replica, value = sum over ranks, scaling = "weak".
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_DW = 1872            # flop/site, Dw or Dw^+ with clover
+FLOP_DHAT = 1848          # flop per lattice site, even-odd operator
+REALS_DW = {18: 192, 12: 168}      # compulsory reals/site per application
+REALS_DHAT = {18: 276, 12: 228}    # even-odd operator (two half hops touch every link once each)
+REALS_CG_ITER = {18: 528, 12: 480}  # fused CG iteration
+NOMINAL_HBM_GBS = 8000.0  # the figure north_star quotes
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lattice", default="48x48x48x96", help="L1xL2xL3xL4 of the timed workload")
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--no-rows", action="store_true", help="skip the per-row extras (rank 0, N=1)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--kappa", type=float, default=0.137)
+    ap.add_argument("--csw", type=float, default=1.9)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU with NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.01):
+        threading.Thread.__init__(self, daemon=True)
+        self.index, self.period = index, period
+        self.stop_flag = threading.Event()
+        self.sm, self.reasons, self.sm_max, self.err = [], set(), None, None
+
+    def run(self):
+        try:
+            import pynvml as N
+            N.nvmlInit()
+            h = N.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = int(N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM))
+            names = {
+                getattr(N, "nvmlClocksEventReasonGpuIdle", 0x1): "gpu_idle",
+                getattr(N, "nvmlClocksEventReasonApplicationsClocksSetting", 0x2): "applications_clocks_setting",
+                getattr(N, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+                getattr(N, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(N, "nvmlClocksEventReasonSyncBoost", 0x10): "sync_boost",
+                getattr(N, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(N, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(N, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+            }
+            while not self.stop_flag.is_set():
+                self.sm.append(int(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM)))
+                try:
+                    r = int(N.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    r = int(N.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                for bit, name in names.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+                time.sleep(self.period)
+        except Exception as e:  # NVML missing: report, do not invent numbers
+            self.err = repr(e)
+
+    def result(self):
+        self.stop_flag.set()
+        self.join(timeout=2.0)
+        sm = sorted(self.sm)
+        out = {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+               "samples": len(sm)}
+        if self.err:
+            out["error"] = self.err
+        return out
+
+
+# ------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def time_calls(torch, fn, reps, warm=2):
+    """Average milliseconds of fn() over `reps` back-to-back calls (CUDA events on the current stream)."""
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+class Setup:
+    """Synthetic gauge field + clover term + spinors of one lattice, resident in HBM in the internal layout."""
+
+    def __init__(self, torch, B, synth, L, bc, theta, phiT, kappa, csw, seed_cfg, rank, precs, recons, inverse=False,
+                 sf=False, keep_canon=False):
+        self.torch, self.B, self.L, self.kappa, self.csw = torch, B, tuple(L), kappa, csw
+        self.V = synth.vol(L)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.g = B.geom_create(L, bc, theta, synth.SF_PHI0 if sf else None, phiT, device=dev.index)
+        Uc = synth.smooth_gauge_torch(L, synth.seed_for(seed_cfg, 0) + 100 * rank, dev)
+        if sf:
+            n0 = L[0] * L[1] * L[2]
+            for mu in range(3):
+                Uc[:n0, mu] = torch.from_numpy(synth.sf_boundary_links(L, synth.SF_PHI0, mu)).to(dev)
+        psic = synth.gaussian_spinor_torch(L, synth.seed_for(seed_cfg, 1) + 100 * rank, dev)
+        self.U, self.A, self.Ainv, self.psi, self.out = {}, {}, {}, {}, {}
+        for recon in recons:
+            for prec in sorted(set(precs) | {B.F64}):
+                buf = B.alloc_field(self.g, B.FIELD_GAUGE, prec, recon)
+                B.gauge_import(self.g, Uc, buf, prec, recon)
+                self.U[(prec, recon)] = buf
+        r0 = recons[0]
+        for prec in precs:
+            A = B.alloc_field(self.g, B.FIELD_CLOVER, prec)
+            Ai = B.alloc_field(self.g, B.FIELD_CLOVER, prec) if inverse else None
+            self.clover_ms = time_calls(
+                torch, lambda: B.clover_build(self.g, kappa, csw, self.U[(B.F64, r0)], A, Ai, r0, prec), 1, 0)
+            self.A[prec], self.Ainv[prec] = A, Ai
+            self.psi[prec] = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
+            self.out[prec] = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
+            B.spinor_import(self.g, psic, self.psi[prec], prec)
+        torch.cuda.synchronize()
+        self.canon = (Uc, psic) if keep_canon else None
+
+    def close(self):
+        self.B.geom_destroy(self.g)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+
+    from paper_2503_16994_b200 import binding as B
+    from paper_2503_16994_b200 import synth
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU fallback")
+    B.lib()  # fails loudly if the extension is missing
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    L = tuple(int(v) for v in args.lattice.lower().split("x"))
+    prec = B.F64 if args.prec == "f64" else B.F32
+    recon = args.recon
+    rb = 8 if prec == B.F64 else 4
+    want_e2e = not args.no_e2e
+    S = Setup(torch, B, synth, L, B.BC_PERIODIC, None, None, args.kappa, args.csw, 5, rank, [prec], [recon],
+              keep_canon=True)
+    V = S.V
+    U, A, psi, out = S.U[(prec, recon)], S.A[prec], S.psi[prec], S.out[prec]
+    out2 = B.alloc_field(S.g, B.FIELD_SPINOR, prec)
+
+    def step():
+        B.dw_apply(S.g, args.kappa, U, A, psi, out, prec, recon)
+        B.dwdag_apply(S.g, args.kappa, U, A, out, out2, prec, recon)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.05)
+    l0 = B.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    launches = B.launch_count() - l0
+    ms_local = e0.elapsed_time(e1)
+    clocks = sampler.result()
+    barrier()
+    ms = ms_local
+    if dist is not None:
+        t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    flops_step = 2.0 * FLOP_DW * V
+    value = world * flops_step / (ms_per_step * 1e-3) / 1e9  # GFLOP/s, whole job
+
+    # roofline of the dominant kernel (the stencil), from this rank's own launches in the timed region
+    peak, peak_src = measured_peaks()
+    bytes_launch = REALS_DW[recon] * rb * V
+    ms_launch = ms_local / launches
+    achieved = bytes_launch / (ms_launch * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "dw_kernel", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "peak_source": peak_src,
+                "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
+                "bytes_per_launch": bytes_launch, "ms_per_launch": round(ms_launch, 4),
+                "model": "%d reals/site compulsory (links + psi in + psi out + clover), each datum once" % REALS_DW[recon],
+                "traffic": NCU_TRAFFIC.get((args.lattice, args.prec, recon))}
+
+    # e2e: same metric through the host-buffer C-ABI call, H2D and D2H inside the timed region
+    e2e = None
+    if want_e2e:
+        e2e = run_e2e(torch, B, S, args, L, prec, recon, dist)
+    result = {
+        "metric": "Dw GFLOP/s (clover Wilson-Dirac, 1872 flop/site/application)", "value": round(value, 1),
+        "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.prec, "data": "synthetic",
+        "config": {"workload": "Dw^+Dw application, %s periodic SU(3), smooth links plaq~0.6, kappa=%g csw=%g, recon=%d"
+                               % (args.lattice, args.kappa, args.csw, recon),
+                   "step": "1 lqcd_dw_apply + 1 lqcd_dwdag_apply on a fixed Gaussian spinor",
+                   "l2": "inputs larger than L2 (%.1f GB compulsory per application), no flush" % (bytes_launch / 1e9),
+                   "parallelism": "replicas x%d (no data-path collective)" % world},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "e2e": e2e,
+    }
+    if rank == 0 and world == 1:
+        if not args.no_rows:
+            result["rows"] = run_rows(torch, B, synth, S, args, prec, recon, peak)
+        if not args.no_cpu:
+            result["cpu_baseline"] = cpu_baseline(np, torch, S, args)
+    S.close()
+    if rank == 0:
+        print(json.dumps(result))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of dw_kernel from the committed ncu --set full
+# capture (profiles/); keyed by (lattice, prec, recon).  None = not captured for that configuration.
+NCU_TRAFFIC = {}
+
+
+def run_e2e(torch, B, S, args, L, prec, recon, dist):
+    """lqcd_dw_apply_host: canonical HOST buffers in, canonical HOST buffer out; every call copies the gauge
+    field and the spinor to the device, converts the layout, builds the clover term, applies Dw, converts back
+    and copies the result to the host.  Pinned host memory; wall clock around the (synchronous) call."""
+    Uc, psic = S.canon
+    V = S.V
+    hU = torch.empty(Uc.shape, dtype=Uc.dtype, pin_memory=True)
+    hpsi = torch.empty(psic.shape, dtype=psic.dtype, pin_memory=True)
+    hout = torch.empty(psic.shape, dtype=psic.dtype, pin_memory=True)
+    hU.copy_(Uc)
+    hpsi.copy_(psic)
+    torch.cuda.synchronize()
+    S.canon = None
+    del Uc, psic
+    torch.cuda.empty_cache()
+    n = max(1, min(args.steps, 3))
+
+    def call():
+        B.dw_apply_host(L, args.kappa, args.csw, hU, hpsi, hout, prec=prec, recon=recon,
+                        device=torch.cuda.current_device())
+
+    call()  # warm-up (first-touch of the driver's staging paths)
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(n):
+        call()
+    dt = (time.perf_counter() - t0) / n
+    world = 1
+    if dist is not None:
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        world = dist.get_world_size()
+    h2d = int(hU.numel() * 16 + hpsi.numel() * 16)
+    d2h = int(hout.numel() * 16)
+    return {"value": round(world * FLOP_DW * V / dt / 1e9, 2), "unit": "GFLOP/s", "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "ms_per_step": round(dt * 1e3, 2), "steps": n,
+            "api": "lqcd_dw_apply_host (one Dw application per call: H2D gauge+spinor, layout import, Csw!, Dw, export, D2H)",
+            "checksum": float(hout.real.abs().sum().item()) if V <= (1 << 22) else None}
+
+
+def run_rows(torch, B, synth, S, args, prec, recon, peak):
+    """The other hot-path rows measured once each, same process, rank 0, N = 1."""
+    rows = {}
+    V, L, g, kappa = S.V, S.L, S.g, args.kappa
+
+    def gbs(reals, rbytes, ms, sites=V):
+        return round(reals * rbytes * sites / (ms * 1e-3) / 1e9, 1)
+
+    rows["a3_clover_build"] = {"ms": round(S.clover_ms, 3), "lattice": args.lattice,
+                               "GB/s_model": gbs(144, 8, S.clover_ms),
+                               "model": "read 72 link reals + write 72 clover reals per site, fp64"}
+    # a4: Dw in every precision / link format
+    dw = {}
+    for p, pname, rb in ((B.F64, "f64", 8), (B.F32, "f32", 4)):
+        if p not in S.A:
+            A = B.alloc_field(g, B.FIELD_CLOVER, p)
+            B.clover_build(g, kappa, args.csw, S.U[(B.F64, recon)], A, None, recon, p)
+            S.A[p] = A
+            S.psi[p] = B.alloc_field(g, B.FIELD_SPINOR, p)
+            S.out[p] = B.alloc_field(g, B.FIELD_SPINOR, p)
+            if p == B.F32:
+                B.field_to_f32(g, B.FIELD_SPINOR, recon, S.psi[B.F64], S.psi[p])
+        for r in (18, 12):
+            if (p, r) not in S.U:
+                if (B.F64, r) not in S.U:
+                    # derive the 12-real field from the 18-real one through the canonical layout
+                    canon = torch.empty((V, 4, 3, 3), dtype=torch.complex128, device="cuda")
+                    B.gauge_export(g, S.U[(B.F64, recon)], canon, B.F64, recon)
+                    S.U[(B.F64, r)] = B.alloc_field(g, B.FIELD_GAUGE, B.F64, r)
+                    B.gauge_import(g, canon, S.U[(B.F64, r)], B.F64, r)
+                    del canon
+                if p == B.F32:
+                    S.U[(p, r)] = B.alloc_field(g, B.FIELD_GAUGE, p, r)
+                    B.field_to_f32(g, B.FIELD_GAUGE, r, S.U[(B.F64, r)], S.U[(p, r)])
+            for dag, fn in (("dw", B.dw_apply), ("dwdag", B.dwdag_apply)):
+                ms = time_calls(torch, lambda: fn(g, kappa, S.U[(p, r)], S.A[p], S.psi[p], S.out[p], p, r), 10)
+                dw["%s_%s_recon%d" % (dag, pname, r)] = {
+                    "ms": round(ms, 4), "GFLOP/s": round(FLOP_DW * V / ms / 1e6, 1), "GB/s": gbs(REALS_DW[r], rb, ms),
+                    "frac_measured_peak": round(gbs(REALS_DW[r], rb, ms) / peak, 4)}
+    rows["a4_dw"] = dw
+    # a6: BLAS-1 reduction alone (|v|^2 over one spinor)
+    ws = B.alloc_field(g, B.FIELD_WORKSPACE)
+    ms = time_calls(torch, lambda: B.spinor_norm2(g, S.psi[B.F64], ws), 10)
+    rows["a6_norm2_f64"] = {"ms": round(ms, 4), "GB/s": gbs(24, 8, ms), "frac_measured_peak": round(gbs(24, 8, ms) / peak, 4)}
+    # a7: CG iteration rate on the bench lattice (fixed iteration counts; the difference removes set-up cost)
+    b, x = S.psi[B.F64], S.out[B.F64]
+    t = {}
+    for n in (10, 40):
+        info = B.cg_solve(g, kappa, S.U[(B.F64, recon)], S.A[B.F64], b, x, ws, tol=1e-30, maxiter=n, check_every=n,
+                          recon=recon, raise_on_notconv=False)
+        t[n] = info["seconds"]
+    ms_it = (t[40] - t[10]) / 30 * 1e3
+    rows["a7_cg_iteration_f64"] = {"ms_per_iteration": round(ms_it, 4), "lattice": args.lattice,
+                                   "GB/s_model": gbs(REALS_CG_ITER[recon], 8, ms_it),
+                                   "frac_measured_peak": round(gbs(REALS_CG_ITER[recon], 8, ms_it) / peak, 4),
+                                   "model": "%d reals/site/iteration (fused plan, SURVEY.md 8(d))" % REALS_CG_ITER[recon]}
+    del ws
+    torch.cuda.empty_cache()
+    rows.update(run_config3(torch, B, synth, peak))
+    rows.update(run_config4(torch, B, synth, peak))
+    return rows
+
+
+def run_config3(torch, B, synth, peak):
+    """configs[2]: 24^3 x 48, open BC, 12 point-source columns to 1e-10, fp64 (time-to-solution)."""
+    L, kappa, csw = (24, 24, 24, 48), 0.1365, 1.9
+    S = Setup(torch, B, synth, L, B.BC_OPEN, None, None, kappa, csw, 3, 0, [B.F64, B.F32], [18], inverse=True)
+    g = S.g
+    U32 = B.alloc_field(g, B.FIELD_GAUGE, B.F32, 18)
+    B.field_to_f32(g, B.FIELD_GAUGE, 18, S.U[(B.F64, 18)], U32)
+    ws = B.alloc_field(g, B.FIELD_WORKSPACE)
+    cols = torch.empty(12 * B.field_bytes(g, B.FIELD_SPINOR), dtype=torch.uint8, device="cuda")
+    y = (0, 0, 0, L[3] // 2)   # R12: slice 0 is frozen under open BC
+    out = {}
+    for name, kw in (("plain_f64", {}),
+                     ("eo_mixed", dict(eo=True, mixed=True, clover_inv64=S.Ainv[B.F64], U32=U32, clover32=S.A[B.F32],
+                                       clover_inv32=S.Ainv[B.F32]))):
+        t0 = time.perf_counter()
+        infos = B.propagator(g, kappa, S.U[(B.F64, 18)], S.A[B.F64], y, cols, ws, tol=1e-10, maxiter=10000, **kw)
+        dt = time.perf_counter() - t0
+        out["a8_propagator_24x24x24x48_open_" + name] = {
+            "seconds_12_columns": round(dt, 3), "iterations": [i["iters"] for i in infos],
+            "max_rel_resid_normal": max(i["rel_resid_normal"] for i in infos),
+            "max_rel_resid_true": max(i["rel_resid_true"] for i in infos)}
+    S.close()
+    del S, cols, ws, U32
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_config4(torch, B, synth, peak):
+    """configs[3]: 32^3 x 64, SF BC, theta = 0.5 spatial: even-odd operator throughput fp64 vs fp32, mixed CG."""
+    L, kappa, csw = (32, 32, 32, 64), 0.1355, 1.8
+    theta = (0.5, 0.5, 0.5, 0.0)
+    S = Setup(torch, B, synth, L, B.BC_SF_ORBI, theta, synth.SF_PHIT, kappa, csw, 4, 0, [B.F64, B.F32], [18],
+              inverse=True, sf=True)
+    g, V = S.g, S.V
+    U32 = B.alloc_field(g, B.FIELD_GAUGE, B.F32, 18)
+    B.field_to_f32(g, B.FIELD_GAUGE, 18, S.U[(B.F64, 18)], U32)
+    S.U[(B.F32, 18)] = U32
+    out = {}
+    for p, pname, rb in ((B.F64, "f64", 8), (B.F32, "f32", 4)):
+        tmp = B.alloc_field(g, B.FIELD_SPINOR, p)
+        ms = time_calls(torch, lambda: B.dw_eo_apply(g, kappa, S.U[(p, 18)], S.A[p], S.Ainv[p], S.psi[p], S.out[p], tmp,
+                                                     False, p, 18), 20)
+        gb = REALS_DHAT[18] * rb * V / (ms * 1e-3) / 1e9
+        out["a5_dhat_32x32x32x64_sf_" + pname] = {"ms": round(ms, 4), "GFLOP/s": round(FLOP_DHAT * V / ms / 1e6, 1),
+                                                  "GB/s": round(gb, 1), "frac_measured_peak": round(gb / peak, 4)}
+    ws = B.alloc_field(g, B.FIELD_WORKSPACE)
+    y = (0, 0, 0, L[3] // 2)
+    b = B.alloc_field(g, B.FIELD_SPINOR)
+    x = B.alloc_field(g, B.FIELD_SPINOR)
+    B.point_source(g, y, 0, 0, b)
+    for name, kw in (("eo_f64", dict(eo=True)), ("eo_mixed", dict(eo=True, mixed=True))):
+        info = B.cg_solve(g, kappa, S.U[(B.F64, 18)], S.A[B.F64], b, x, ws, tol=1e-10, maxiter=10000,
+                          clover_inv64=S.Ainv[B.F64], U32=U32, clover32=S.A[B.F32], clover_inv32=S.Ainv[B.F32], **kw)
+        out["a7_cg_32x32x32x64_sf_" + name] = {k: info[k] for k in ("iters", "outer", "seconds", "rel_resid_normal", "rel_resid_true")}
+    S.close()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and the --impl reference arm
+# ------------------------------------------------------------------------------------------------------
+SAMPLE_L = (16, 16, 16, 32)
+
+
+def oracle_sample_inputs(np, synth, args, U_canon_dev=None, psi_canon_dev=None, L_full=None):
+    """A 16^3 x 32 periodic sample of the bench workload.  Links of the recipe are independent, so any
+    sub-block of the bench field is a field of the same recipe; without a device field, draw one on the host."""
+    L = SAMPLE_L
+    if U_canon_dev is not None:
+        Lf = L_full
+        U4 = U_canon_dev.reshape(Lf[3], Lf[2], Lf[1], Lf[0], 4, 3, 3)[:L[3], :L[2], :L[1], :L[0]]
+        p4 = psi_canon_dev.reshape(Lf[3], Lf[2], Lf[1], Lf[0], 4, 3)[:L[3], :L[2], :L[1], :L[0]]
+        U = U4.contiguous().reshape(-1, 4, 3, 3).cpu().numpy()
+        psi = p4.contiguous().reshape(-1, 4, 3).cpu().numpy()
+    else:
+        U = synth.smooth_gauge(L, synth.seed_for(5, 0))
+        psi = synth.gaussian_spinor(L, synth.seed_for(5, 1))
+    return L, U, psi
+
+
+def time_oracle(np, oracle, L, U, psi, kappa, csw, budget_s, min_steps=1, max_steps=None, warm=1):
+    """Time steps of (Dw, Dw^+) with the oracle as it stands; returns (GFLOP/s, steps, seconds, threads)."""
+    V = int(np.prod(L))
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    for _ in range(warm):
+        oracle.dw(L, U, oracle.dw(L, U, psi, kappa, A), kappa, A, dagger=True)
+    steps, t0 = 0, time.perf_counter()
+    while True:
+        oracle.dw(L, U, oracle.dw(L, U, psi, kappa, A), kappa, A, dagger=True)
+        steps += 1
+        dt = time.perf_counter() - t0
+        if max_steps is not None and steps >= max_steps:
+            break
+        if max_steps is None and steps >= min_steps and dt >= budget_s:
+            break
+    return 2.0 * FLOP_DW * V * steps / dt / 1e9, steps, dt, oracle.num_threads()
+
+
+def cpu_baseline(np, torch, S, args):
+    import oracle
+    from paper_2503_16994_b200 import synth
+
+    if S.canon is not None:
+        L, U, psi = oracle_sample_inputs(np, synth, args, S.canon[0], S.canon[1], S.L)
+    else:
+        L, U, psi = oracle_sample_inputs(np, synth, args)
+    v, steps, dt, threads = time_oracle(np, oracle, L, U, psi, args.kappa, args.csw, budget_s=10.0)
+    return {"value": round(v, 3), "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+            "sample": "%d steps (Dw then Dw^+, fp64, clover blocks precomputed) on a %s periodic lattice of the bench "
+                      "recipe (kappa=%g csw=%g), %.1f s" % (steps, "x".join(map(str, L)), args.kappa, args.csw, dt)}
+
+
+def run_reference(args):
+    """--impl reference: there is no reference code (PAPER.md only); the arm is the fp64 oracle on the host cores."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import numpy as np
+
+    import oracle
+    from paper_2503_16994_b200 import synth
+
+    L, U, psi = oracle_sample_inputs(np, synth, args)
+    V = int(np.prod(L))
+    steps = max(1, args.steps)
+    v, steps, dt, threads = time_oracle(np, oracle, L, U, psi, args.kappa, args.csw, budget_s=0.0, max_steps=steps,
+                                        warm=max(1, min(args.warmup, 3)))
+    sample = ("each step = Dw then Dw^+ (fp64, clover blocks precomputed) on a %s periodic sample of the bench recipe"
+              % "x".join(map(str, L)))
+    print(json.dumps({
+        "impl": "reference", "metric": "Dw GFLOP/s (clover Wilson-Dirac, 1872 flop/site/application)",
+        "value": round(v, 3), "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": steps, "warmup": max(1, min(args.warmup, 3)),
+        "ms_per_step": round(dt / steps * 1e3, 2), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "Dw^+Dw application, %s periodic SU(3), smooth links plaq~0.6, kappa=%g csw=%g, recon=18"
+                               % (args.lattice, args.kappa, args.csw), "sample": sample},
+        "cpu_baseline": {"value": round(v, 3), "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": round(v, 3), "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
