@@ -8,6 +8,7 @@
 
 #include <atomic>
 #include <chrono>
+#include <vector>
 
 #include "cg.cuh"
 
@@ -189,12 +190,40 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device), "cudaGetDeviceProperties");
   h->sm_count = prop.multiProcessorCount;
+  h->smem_optin = (int)prop.sharedMemPerBlockOptin;
+  g.sm_count = h->sm_count;
+  g.smem_optin = h->smem_optin;
+  {  // neighbour-tile table (a1): 8 neighbours + time origin per tile
+    std::vector<int> tab((size_t)g.ntiles * TILE_TAB, 0);
+    for (int t = 0; t < g.ntiles; t++) {
+      int Tc[4];
+      tile_coords(g, t, Tc);
+      for (int mu = 0; mu < 4; mu++)
+        for (int d = 0; d < 2; d++) {
+          int Tn[4] = {Tc[0], Tc[1], Tc[2], Tc[3]};
+          Tn[mu] += d ? -1 : +1;
+          if (Tn[mu] < 0) Tn[mu] += g.nt[mu];
+          if (Tn[mu] >= g.nt[mu]) Tn[mu] -= g.nt[mu];
+          tab[(size_t)t * TILE_TAB + 2 * mu + d] = tile_linear(g, Tn[0], Tn[1], Tn[2], Tn[3]);
+        }
+      tab[(size_t)t * TILE_TAB + 8] = Tc[3] * g.b[3];
+    }
+    int* dtab = nullptr;
+    if (!cuda_ok(cudaMalloc(&dtab, tab.size() * sizeof(int)), "cudaMalloc(tile table)")) { free(h); return LQCD_ENOMEM; }
+    if (!cuda_ok(cudaMemcpy(dtab, tab.data(), tab.size() * sizeof(int), cudaMemcpyHostToDevice), "cudaMemcpy(tile table)")) {
+      cudaFree(dtab); free(h); return LQCD_ECUDA;
+    }
+    g.tile_tab = dtab;
+  }
   *out = h;
   return LQCD_OK;
 }
 
 lqcd_status lqcd_geom_destroy(lqcd_geom* g) {
-  if (g) free(g);
+  if (g) {
+    if (g->g.tile_tab) cudaFree((void*)g->g.tile_tab);
+    free(g);
+  }
   return LQCD_OK;
 }
 

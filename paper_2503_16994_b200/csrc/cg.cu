@@ -81,7 +81,8 @@ cudaError_t cg_normal(const Op<T>& M, const void* bprime, void* x, const CgVecto
                       int check_every, CgState* host_state, cudaStream_t s) {
   const size_t n = M.ncomplex();
   const size_t bytes = n * sizeof(T2<T>);
-  const int nt = M.geom->g.ntiles;
+  const int nt = M.eo ? dw_num_partials<T>(M.geom->g, M.recon, DIAG_PRE, 0)
+                      : dw_num_partials<T>(M.geom->g, M.recon, M.A ? DIAG_PRE : DIAG_ONE, -1);
   CK(cudaMemsetAsync(x, 0, bytes, s));
   CK(cudaMemcpyAsync(v.r, bprime, bytes, cudaMemcpyDeviceToDevice, s));
   CK(cudaMemcpyAsync(v.p, bprime, bytes, cudaMemcpyDeviceToDevice, s));

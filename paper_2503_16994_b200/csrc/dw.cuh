@@ -26,6 +26,10 @@ struct DwArgs {
   int epi;
 };
 
+// number of per-CTA partial sums an EPI_*_NORM launch with these arguments writes to DwArgs::partial
+template <typename T>
+int dw_num_partials(const Geom& g, int recon, int diag, int parity);
+
 template <typename T>
 cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cudaStream_t s);
 // out(x) = B(x) in(x) on sites of `parity` (-1: all), zero on frozen slices; B = packed 6x6 blocks

@@ -30,7 +30,13 @@ struct Geom {
   int ntiles;
   int bc;         // lqcd_bc
   long long Vh;   // sites of one parity
+  // device table, TILE_TAB ints per tile: linear index of the 8 neighbour tiles (2*mu + (0: +mu, 1: -mu)),
+  // then the time coordinate of the tile origin (library-owned, built by lqcd_geom_create)
+  const int* tile_tab;
+  int sm_count;     // host-side launch configuration (SMs, opt-in shared memory per CTA)
+  int smem_optin;
 };
+enum { TILE_TAB = 12 };
 
 // ---- tile order: [T2hi][T1hi][T3][T2lo][T1lo][T0] -------------------------------------------------
 __host__ __device__ inline int tile_linear(const Geom& g, int T0, int T1, int T2, int T3) {
@@ -137,4 +143,5 @@ struct lqcd_geom {
   double th_re[4], th_im[4];   // per-link phase factors exp(i theta/L)
   bool has_theta;
   int sm_count;
+  int smem_optin;   // max dynamic shared memory per CTA (opt-in)
 };
