@@ -56,14 +56,19 @@ static bool parse_ints(const char* s, int* out, int n) {
   return true;
 }
 
-// Tile shape: 8x4x4x2 sites (TV = 128 per parity, 256 threads for the full operator) when the extents
-// allow it; smaller powers of two otherwise; a longer time extent of the tile when the spatial one is short.
+// Tile shape: 4x4x4x4 sites (TV = 128 per parity, 256 threads for the full operator) when the extents allow
+// it, else 8x4x4x2; smaller powers of two otherwise; a longer time extent of the tile when the spatial one is short.
 static void choose_tiling(Geom& g) {
   int b[4];
   b[0] = pow2_divisor(g.L[0], 8);
   b[1] = pow2_divisor(g.L[1], 4);
   b[2] = pow2_divisor(g.L[2], 4);
   b[3] = 2;
+  if (g.L[0] % 4 == 0 && g.L[1] % 4 == 0 && g.L[2] % 4 == 0 && g.L[3] % 4 == 0) {
+    // 4^4: the smallest surface (512 halo sites per 256) and four equal faces, which is what lets the
+    // double-buffered halo area of the persistent kernel fit shared memory in fp64
+    b[0] = b[1] = b[2] = b[3] = 4;
+  }
   int env[4];
   if (parse_ints(getenv("LQCD_TILE"), env, 4)) {
     bool ok = true;
@@ -189,6 +194,13 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   }
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device), "cudaGetDeviceProperties");
+  if (getenv("LQCD_L2_FETCH")) {   // experiment: DRAM -> L2 fetch granularity hint (32/64/128 bytes)
+    size_t before = 0, after = 0;
+    cudaDeviceGetLimit(&before, cudaLimitMaxL2FetchGranularity);
+    cudaError_t e = cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)atoi(getenv("LQCD_L2_FETCH")));
+    cudaDeviceGetLimit(&after, cudaLimitMaxL2FetchGranularity);
+    fprintf(stderr, "[lqcd] L2 fetch granularity %zu -> %zu (%s)\n", before, after, cudaGetErrorString(e));
+  }
   h->sm_count = prop.multiProcessorCount;
   h->smem_optin = (int)prop.sharedMemPerBlockOptin;
   g.sm_count = h->sm_count;

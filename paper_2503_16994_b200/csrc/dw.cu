@@ -12,6 +12,7 @@
 // Epilogues (CG fusion): EPI_STORE, EPI_STORE_NORM (|out|^2 partial per CTA),
 // EPI_AXPY_NORM (r -= alpha*out, |r|^2 partial; out itself is never written).
 #include <stdlib.h>
+#include <string.h>
 
 #include "dw.cuh"
 #include "pipe.cuh"
@@ -35,13 +36,14 @@ __device__ __forceinline__ cx<T> ldx(const T2<T>* p) {
 //   mu=2: h0 = p0 + m i p2, h1 = p1 - m i p3; low2 = -m i y0, low3 = +m i y1
 //   mu=3: h0 = p0 - m p2,   h1 = p1 - m p3;   low2 = -m y0,   low3 = -m y1
 template <typename T, int RECON, int MU, bool FWD, bool LDG = true>
-__device__ __forceinline__ void hop_dir(const T2<T>* __restrict__ psi, const T2<T>* __restrict__ u, const int TV,
-                                        const T m, const bool has_theta, const cx<T> th, cx<T> (&acc)[12]) {
+__device__ __forceinline__ void hop_dir(const T2<T>* __restrict__ psi, const T2<T>* __restrict__ u, const int SP,
+                                        const int SU, const T m, const bool has_theta, const cx<T> th,
+                                        cx<T> (&acc)[12]) {
   cx<T> h[2][3];
 #pragma unroll
   for (int a = 0; a < 3; a++) {
-    cx<T> p0 = ldx<T, LDG>(psi + (0 + a) * TV), p1 = ldx<T, LDG>(psi + (3 + a) * TV);
-    cx<T> p2 = ldx<T, LDG>(psi + (6 + a) * TV), p3 = ldx<T, LDG>(psi + (9 + a) * TV);
+    cx<T> p0 = ldx<T, LDG>(psi + (0 + a) * SP), p1 = ldx<T, LDG>(psi + (3 + a) * SP);
+    cx<T> p2 = ldx<T, LDG>(psi + (6 + a) * SP), p3 = ldx<T, LDG>(psi + (9 + a) * SP);
     if (MU == 0) {
       h[0][a] = cx<T>(fma(-m, p3.im, p0.re), fma(m, p3.re, p0.im));
       h[1][a] = cx<T>(fma(-m, p2.im, p1.re), fma(m, p2.re, p1.im));
@@ -60,7 +62,7 @@ __device__ __forceinline__ void hop_dir(const T2<T>* __restrict__ psi, const T2<
 #pragma unroll
   for (int i = 0; i < (RECON == 12 ? 2 : 3); i++)
 #pragma unroll
-    for (int k = 0; k < 3; k++) U[i][k] = ldx<T, LDG>(u + (3 * i + k) * TV);
+    for (int k = 0; k < 3; k++) U[i][k] = ldx<T, LDG>(u + (3 * i + k) * SU);
   if (RECON == 12) {  // row 3 = conj(row 1 x row 2) (R16)
     U[2][0] = conj(U[0][1] * U[1][2] - U[0][2] * U[1][1]);
     U[2][1] = conj(U[0][2] * U[1][0] - U[0][0] * U[1][2]);
@@ -136,152 +138,145 @@ __device__ __forceinline__ void clover_mul(const T2<T>* __restrict__ A, const in
   }
 }
 
-template <typename T, int RECON, int DIAG>
-__global__ void __launch_bounds__(256) dw_kernel(const Geom g, const DwArgs<T> a) {
+// One thread per site, one tile (both parities for the full operator) per CTA at a time; CTA b works through
+// tiles b, b + gridDim.x, ... (gridDim.x == ntiles gives the plain one-tile-per-CTA launch).
+template <typename T, int RECON, int DIAG, bool SPLIT>
+__device__ __forceinline__ void dw_body(const Geom& g, const DwArgs<T>& a) {
   constexpr int NCU = (RECON == 12) ? 6 : 9;
-  __shared__ int s_nbr[8];
   __shared__ double s_red[8];
   if (a.skip != nullptr && *a.skip != 0) return;  // CG finished: uniform early exit
   const int TV = g.TV;
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x;
-  int Tc[4];
-  tile_coords(g, tile, Tc);
-  if (tid < 8) {
-    int mu = tid >> 1, d = (tid & 1) ? -1 : +1;
-    int Tn[4] = {Tc[0], Tc[1], Tc[2], Tc[3]};
-    Tn[mu] += d;
-    if (Tn[mu] < 0) Tn[mu] += g.nt[mu];
-    if (Tn[mu] >= g.nt[mu]) Tn[mu] -= g.nt[mu];
-    s_nbr[tid] = tile_linear(g, Tn[0], Tn[1], Tn[2], Tn[3]);
-  }
-  __syncthreads();
-
-  const int npar = (a.parity < 0) ? 2 : 1;
+  // SPLIT: the full operator with one PARITY of a tile per CTA (work item = 2*tile + parity, TV threads): three
+  // 128-thread CTAs fit an SM where one 256-thread CTA did, i.e. 12 warps of loads in flight instead of 8.
+  const int npar = (!SPLIT && a.parity < 0) ? 2 : 1;
   const bool active = tid < npar * TV;
-  const int pidx = (tid >= TV) ? 1 : 0;
-  const int j = tid - pidx * TV;
+  const int pidx = SPLIT ? (int)(blockIdx.x & 1) : ((tid >= TV) ? 1 : 0);
+  const int j = SPLIT ? tid : tid - pidx * TV;
   const int p = (a.parity < 0) ? pidx : a.parity;
+  const int q = 1 - p;
   double nrm = 0.0;
-
-  if (active) {
-    int l[4];
-    local_coords(g, j, p, l);
-    const int x3 = Tc[3] * g.b[3] + l[3];
-    const bool nonper = (g.bc != LQCD_BC_PERIODIC);
-    const bool fz = nonper && frozen_slice(g, x3);
-    cx<T> res[12];
-    if (fz) {
+  int l[4];
+  local_coords(g, j, p, l);
+  const bool nonper = (g.bc != LQCD_BC_PERIODIC);
+  const T sg = a.dagger ? T(-1) : T(1);
+  const int bh0 = g.b[0] >> 1;
+  const int l0h = l[0] >> 1;
+  const int st1 = bh0, st2 = bh0 << g.lb[1], st3 = st2 << g.lb[2];
+  const int tstep = SPLIT ? (int)(gridDim.x >> 1) : (int)gridDim.x;   // SPLIT needs an even grid
+  for (int tile = SPLIT ? (int)(blockIdx.x >> 1) : (int)blockIdx.x; tile < g.ntiles; tile += tstep) {
+    const int* __restrict__ tab = g.tile_tab + (size_t)tile * TILE_TAB;
+    if (active) {
+      const int x3 = __ldg(tab + 8) + l[3];
+      const bool fz = nonper && frozen_slice(g, x3);
+      cx<T> res[12];
+      if (fz) {
 #pragma unroll
-      for (int c = 0; c < 12; c++) res[c] = cx<T>(0, 0);
-    } else {
-      cx<T> acc[12];
-#pragma unroll
-      for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
-      const T sg = a.dagger ? T(-1) : T(1);
-      const int bh0 = g.b[0] >> 1;
-      const int l0h = l[0] >> 1;
-      const int st1 = bh0, st2 = bh0 << g.lb[1], st3 = st2 << g.lb[2];
-      const size_t ubase_self = field_offset(g, 4 * NCU, p, tile, 0, j);
-      const int q = 1 - p;
-      // direction 0
-      {
-        bool cr = (l[0] + 1 == g.b[0]);
-        int jn = j - l0h + (cr ? 0 : ((l[0] + 1) >> 1));
-        int tn = cr ? s_nbr[0] : tile;
-        hop_dir<T, RECON, 0, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(0 * NCU) * TV,
-                                   TV, sg, a.has_theta, a.theta[0], acc);
-        cr = (l[0] == 0);
-        jn = j - l0h + (cr ? bh0 - 1 : ((l[0] - 1) >> 1));
-        tn = cr ? s_nbr[1] : tile;
-        hop_dir<T, RECON, 0, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
-                                    a.U + field_offset(g, 4 * NCU, q, tn, 0 * NCU, jn), TV, -sg, a.has_theta,
-                                    a.theta[0], acc);
-      }
-      // direction 1
-      {
-        bool cr = (l[1] + 1 == g.b[1]);
-        int jn = cr ? j - (g.b[1] - 1) * st1 : j + st1;
-        int tn = cr ? s_nbr[2] : tile;
-        hop_dir<T, RECON, 1, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(1 * NCU) * TV,
-                                   TV, sg, a.has_theta, a.theta[1], acc);
-        cr = (l[1] == 0);
-        jn = cr ? j + (g.b[1] - 1) * st1 : j - st1;
-        tn = cr ? s_nbr[3] : tile;
-        hop_dir<T, RECON, 1, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
-                                    a.U + field_offset(g, 4 * NCU, q, tn, 1 * NCU, jn), TV, -sg, a.has_theta,
-                                    a.theta[1], acc);
-      }
-      // direction 2
-      {
-        bool cr = (l[2] + 1 == g.b[2]);
-        int jn = cr ? j - (g.b[2] - 1) * st2 : j + st2;
-        int tn = cr ? s_nbr[4] : tile;
-        hop_dir<T, RECON, 2, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(2 * NCU) * TV,
-                                   TV, sg, a.has_theta, a.theta[2], acc);
-        cr = (l[2] == 0);
-        jn = cr ? j + (g.b[2] - 1) * st2 : j - st2;
-        tn = cr ? s_nbr[5] : tile;
-        hop_dir<T, RECON, 2, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
-                                    a.U + field_offset(g, 4 * NCU, q, tn, 2 * NCU, jn), TV, -sg, a.has_theta,
-                                    a.theta[2], acc);
-      }
-      // direction 3 (time): hops onto frozen slices are skipped, never multiplied by zero (D7, P7)
-      {
-        bool cr = (l[3] + 1 == g.b[3]);
-        int jn = cr ? j - (g.b[3] - 1) * st3 : j + st3;
-        int tn = cr ? s_nbr[6] : tile;
-        int xn = (x3 + 1 == g.L[3]) ? 0 : x3 + 1;
-        if (!(nonper && frozen_slice(g, xn)))
-          hop_dir<T, RECON, 3, true>(a.in + field_offset(g, 12, q, tn, 0, jn),
-                                     a.U + ubase_self + (size_t)(3 * NCU) * TV, TV, sg, a.has_theta, a.theta[3], acc);
-        cr = (l[3] == 0);
-        jn = cr ? j + (g.b[3] - 1) * st3 : j - st3;
-        tn = cr ? s_nbr[7] : tile;
-        xn = (x3 == 0) ? g.L[3] - 1 : x3 - 1;
-        if (!(nonper && frozen_slice(g, xn)))
-          hop_dir<T, RECON, 3, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
-                                      a.U + field_offset(g, 4 * NCU, q, tn, 3 * NCU, jn), TV, -sg, a.has_theta,
-                                      a.theta[3], acc);
-      }
-      // site-diagonal part
-      if (DIAG == DIAG_POST) {
-        clover_mul<T>(a.A + field_offset(g, 36, p, tile, 0, j), TV, acc, res);
+        for (int c = 0; c < 12; c++) res[c] = cx<T>(0, 0);
       } else {
-        cx<T> v[12];
-        const T2<T>* sp = a.self + field_offset(g, 12, p, tile, 0, j);
+        cx<T> acc[12];
 #pragma unroll
-        for (int c = 0; c < 12; c++) v[c] = ld<T>(sp + c * TV);
-        if (DIAG == DIAG_PRE) {
-          cx<T> av[12];
-          clover_mul<T>(a.A + field_offset(g, 36, p, tile, 0, j), TV, v, av);
-#pragma unroll
-          for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, av[c].re), fma(-a.k, acc[c].im, av[c].im));
+        for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
+        const size_t ubase_self = field_offset(g, 4 * NCU, p, tile, 0, j);
+        // direction 0
+        {
+          bool cr = (l[0] + 1 == g.b[0]);
+          int jn = j - l0h + (cr ? 0 : ((l[0] + 1) >> 1));
+          int tn = cr ? __ldg(tab + 0) : tile;
+          hop_dir<T, RECON, 0, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(0 * NCU) * TV,
+                                     TV, TV, sg, a.has_theta, a.theta[0], acc);
+          cr = (l[0] == 0);
+          jn = j - l0h + (cr ? bh0 - 1 : ((l[0] - 1) >> 1));
+          tn = cr ? __ldg(tab + 1) : tile;
+          hop_dir<T, RECON, 0, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
+                                      a.U + field_offset(g, 4 * NCU, q, tn, 0 * NCU, jn), TV, TV, -sg, a.has_theta,
+                                      a.theta[0], acc);
+        }
+        // direction 1
+        {
+          bool cr = (l[1] + 1 == g.b[1]);
+          int jn = cr ? j - (g.b[1] - 1) * st1 : j + st1;
+          int tn = cr ? __ldg(tab + 2) : tile;
+          hop_dir<T, RECON, 1, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(1 * NCU) * TV,
+                                     TV, TV, sg, a.has_theta, a.theta[1], acc);
+          cr = (l[1] == 0);
+          jn = cr ? j + (g.b[1] - 1) * st1 : j - st1;
+          tn = cr ? __ldg(tab + 3) : tile;
+          hop_dir<T, RECON, 1, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
+                                      a.U + field_offset(g, 4 * NCU, q, tn, 1 * NCU, jn), TV, TV, -sg, a.has_theta,
+                                      a.theta[1], acc);
+        }
+        // direction 2
+        {
+          bool cr = (l[2] + 1 == g.b[2]);
+          int jn = cr ? j - (g.b[2] - 1) * st2 : j + st2;
+          int tn = cr ? __ldg(tab + 4) : tile;
+          hop_dir<T, RECON, 2, true>(a.in + field_offset(g, 12, q, tn, 0, jn), a.U + ubase_self + (size_t)(2 * NCU) * TV,
+                                     TV, TV, sg, a.has_theta, a.theta[2], acc);
+          cr = (l[2] == 0);
+          jn = cr ? j + (g.b[2] - 1) * st2 : j - st2;
+          tn = cr ? __ldg(tab + 5) : tile;
+          hop_dir<T, RECON, 2, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
+                                      a.U + field_offset(g, 4 * NCU, q, tn, 2 * NCU, jn), TV, TV, -sg, a.has_theta,
+                                      a.theta[2], acc);
+        }
+        // direction 3 (time): hops onto frozen slices are skipped, never multiplied by zero (D7, P7)
+        {
+          bool cr = (l[3] + 1 == g.b[3]);
+          int jn = cr ? j - (g.b[3] - 1) * st3 : j + st3;
+          int tn = cr ? __ldg(tab + 6) : tile;
+          int xn = (x3 + 1 == g.L[3]) ? 0 : x3 + 1;
+          if (!(nonper && frozen_slice(g, xn)))
+            hop_dir<T, RECON, 3, true>(a.in + field_offset(g, 12, q, tn, 0, jn),
+                                       a.U + ubase_self + (size_t)(3 * NCU) * TV, TV, TV, sg, a.has_theta, a.theta[3], acc);
+          cr = (l[3] == 0);
+          jn = cr ? j + (g.b[3] - 1) * st3 : j - st3;
+          tn = cr ? __ldg(tab + 7) : tile;
+          xn = (x3 == 0) ? g.L[3] - 1 : x3 - 1;
+          if (!(nonper && frozen_slice(g, xn)))
+            hop_dir<T, RECON, 3, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
+                                        a.U + field_offset(g, 4 * NCU, q, tn, 3 * NCU, jn), TV, TV, -sg, a.has_theta,
+                                        a.theta[3], acc);
+        }
+        // site-diagonal part
+        if (DIAG == DIAG_POST) {
+          clover_mul<T>(a.A + field_offset(g, 36, p, tile, 0, j), TV, acc, res);
         } else {
+          cx<T> v[12];
+          const T2<T>* sp = a.self + field_offset(g, 12, p, tile, 0, j);
 #pragma unroll
-          for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, v[c].re), fma(-a.k, acc[c].im, v[c].im));
+          for (int c = 0; c < 12; c++) v[c] = ld<T>(sp + c * TV);
+          if (DIAG == DIAG_PRE) {
+            cx<T> av[12];
+            clover_mul<T>(a.A + field_offset(g, 36, p, tile, 0, j), TV, v, av);
+#pragma unroll
+            for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, av[c].re), fma(-a.k, acc[c].im, av[c].im));
+          } else {
+#pragma unroll
+            for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, v[c].re), fma(-a.k, acc[c].im, v[c].im));
+          }
         }
       }
-    }
-    // epilogue
-    const size_t ooff = field_offset(g, 12, p, tile, 0, j);
-    if (a.epi == EPI_AXPY_NORM) {
-      const T al = (T)(*a.alpha);
-      T2<T>* rp = a.r + ooff;
+      // epilogue
+      const size_t ooff = field_offset(g, 12, p, tile, 0, j);
+      if (a.epi == EPI_AXPY_NORM) {
+        const T al = (T)(*a.alpha);
+        T2<T>* rp = a.r + ooff;
 #pragma unroll
-      for (int c = 0; c < 12; c++) {
-        T2<T> rv = rp[c * TV];
-        cx<T> w(fma(-al, res[c].re, rv.x), fma(-al, res[c].im, rv.y));
-        st<T>(rp + c * TV, w);
-        nrm += (double)w.re * (double)w.re + (double)w.im * (double)w.im;
-      }
-    } else {
-      T2<T>* op = a.out + ooff;
+        for (int c = 0; c < 12; c++) {
+          T2<T> rv = rp[c * TV];
+          cx<T> w(fma(-al, res[c].re, rv.x), fma(-al, res[c].im, rv.y));
+          st<T>(rp + c * TV, w);
+          nrm += (double)w.re * (double)w.re + (double)w.im * (double)w.im;
+        }
+      } else {
+        T2<T>* op = a.out + ooff;
 #pragma unroll
-      for (int c = 0; c < 12; c++) st<T>(op + c * TV, res[c]);
-      if (a.epi == EPI_STORE_NORM) {
+        for (int c = 0; c < 12; c++) st<T>(op + c * TV, res[c]);
+        if (a.epi == EPI_STORE_NORM) {
 #pragma unroll
-        for (int c = 0; c < 12; c++) nrm += (double)res[c].re * (double)res[c].re + (double)res[c].im * (double)res[c].im;
+          for (int c = 0; c < 12; c++) nrm += (double)res[c].re * (double)res[c].re + (double)res[c].im * (double)res[c].im;
+        }
       }
     }
   }
@@ -299,29 +294,46 @@ __global__ void __launch_bounds__(256) dw_kernel(const Geom g, const DwArgs<T> a
   }
 }
 
+template <typename T, int RECON, int DIAG>
+__global__ void __launch_bounds__(256) dw_kernel(const Geom g, const DwArgs<T> a) {
+  dw_body<T, RECON, DIAG, false>(g, a);
+}
+// 128-thread CTAs (one parity of a tile): three resident per SM
+template <typename T, int RECON, int DIAG, bool SPLIT>
+__global__ void __launch_bounds__(128, 3) dw_kernel_h(const Geom g, const DwArgs<T> a) {
+  dw_body<T, RECON, DIAG, SPLIT>(g, a);
+}
+
 
 // =====================================================================================================
 // Persistent, warp-specialised version of the full-lattice operator (parity = -1, self == in).
 //
-// The direct-load kernel above is latency-bound (184 registers -> 8 warps/SM, every hop a round trip to
-// L2/DRAM).  Here the operands that are streamed from HBM exactly once -- the tile's own links (4 stages of
-// NCU components x both parities), its clover blocks (36/NCU stages) and its spinor -- are fetched by ONE
-// producer lane with 1-D bulk-asynchronous copies (cp.async.bulk, SASS UBLKCP) into a shared-memory ring of
-// `nslot` stage buffers guarded by full/empty mbarriers, so the bytes in flight per SM (nslot-1 stages, ~110 KB
-// in fp64) no longer depend on resident warps.  2*TV consumer threads (one per site, both parities of the
-// tile) run the spin-projected hops and the clover multiply out of shared memory; only neighbours outside
-// the tile and their backward links are read from global memory (L2 hits thanks to the tile order).
-// The tile-blocked layout makes every stage a pair of contiguous blocks, so no tensor map is needed.
+// The one-thread-per-site kernel above is latency-bound: 184 registers per thread in fp64 allow 8 warps per SM
+// and every hop is a dependent round trip to L2/DRAM.  Here NO consumer thread ever touches global memory
+// for its operands; three kinds of warps share a CTA:
+//   * warp 8, one lane: 1-D bulk-asynchronous copies (cp.async.bulk, SASS UBLKCP) stream what a tile reads
+//     from HBM exactly once -- its links (4 stages of NCU components x both parities), its clover blocks
+//     (36/NCU stages) and its spinor -- into a shared-memory ring of `nslot` stage buffers guarded by
+//     full/empty mbarriers.  The tile-blocked layout makes every stage a pair of contiguous blocks, so no
+//     tensor map is needed, and the bytes in flight per SM no longer depend on resident warps.
+//   * warps 9-11: the halo of direction mu -- the spinors on the two faces of the neighbour tiles and the
+//     links U_mu(x - mu) leaving the backward face -- is gathered element by element with per-thread
+//     asynchronous copies (cp.async, SASS LDGSTS; they complete on an mbarrier, occupy no registers) into a
+//     double-buffered halo area; the stage order (below) gives every halo three stages of lead.
+//   * warps 0-7: 2*TV consumer threads, one per site (both parities of the tile), run the spin-projected
+//     hops and the clover multiply purely out of shared memory.
 // =====================================================================================================
 
-// packed Hermitian block, one component at a time: c in [0,36), chirality c/18; slot c%18 < 3 holds two real
-// diagonal entries, slot 3 + i(i-1)/2 + jj the element (i,jj) of the strict lower triangle (D5).
+// packed Hermitian block, one component at a time, ACCUMULATED into o: c in [0,36), chirality c/18; slot
+// c%18 < 3 holds two real diagonal entries, slot 3 + i(i-1)/2 + jj the element (i,jj) of the strict lower
+// triangle (D5).
 template <typename T, int C>
 __device__ __forceinline__ void clover_comp(const cx<T> l, const cx<T> (&v)[12], cx<T> (&o)[12]) {
   constexpr int ch = C / 18, s = C % 18;
-  if (s < 3) {
-    o[6 * ch + 2 * s] = l.re * v[6 * ch + 2 * s];
-    o[6 * ch + 2 * s + 1] = l.im * v[6 * ch + 2 * s + 1];
+  if (s < 3) {   // o += diag * v
+    o[6 * ch + 2 * s] = cx<T>(fma(l.re, v[6 * ch + 2 * s].re, o[6 * ch + 2 * s].re), fma(l.re, v[6 * ch + 2 * s].im, o[6 * ch + 2 * s].im));
+    o[6 * ch + 2 * s + 1] =
+        cx<T>(fma(l.im, v[6 * ch + 2 * s + 1].re, o[6 * ch + 2 * s + 1].re), fma(l.im, v[6 * ch + 2 * s + 1].im, o[6 * ch + 2 * s + 1].im));
   } else {
     constexpr int t = s - 3;
     constexpr int i = (t >= 10) ? 5 : (t >= 6) ? 4 : (t >= 3) ? 3 : (t >= 1) ? 2 : 1;
@@ -343,9 +355,11 @@ struct CloverStage<T, C0, 0> {
   static __device__ __forceinline__ void run(const T2<T>*, const int, const cx<T> (&)[12], cx<T> (&)[12]) {}
 };
 
+enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12 };
 struct PipeBars {
   uint64_t full_sp, empty_sp;
-  uint64_t full[8], empty[8];
+  uint64_t full_h[2], empty_h[2];
+  uint64_t full[PIPE_MAX_SLOTS], empty[PIPE_MAX_SLOTS];
 };
 
 struct RingPos {
@@ -375,17 +389,58 @@ struct CloverPipe<T, NCU, NS, NS> {
                                              const int, const cx<T> (&)[12], cx<T> (&)[12]) {}
 };
 
-// both hops of direction MU for one site, links of the tile in ring stage `ub`, spinor tile in `sp`
+// ---- faces of a tile ------------------------------------------------------------------------------------
+// The sites of one parity on the face l_mu = const of a tile are numbered by their other three coordinates:
+//   mu = 0 : fidx = (l1 >> 1) + (b1/2) * (l2 + b2 * l3)      (l1's low bit is fixed by the parity)
+//   mu >= 1: fidx = l0h + (b0/2) * (la + ba * lb),  (a, b) = the two directions of {1,2,3} other than mu
+// TV / b_mu sites per parity.  A halo buffer for direction mu holds, with Nf = 2*TV/b_mu columns (parity-major):
+//   F [12][Nf]  spinors of the +mu neighbour tile on its face l_mu = 0        (forward hops leaving the tile)
+//   B [12][Nf]  spinors of the -mu neighbour tile on its face l_mu = b_mu - 1 (backward hops leaving the tile)
+//   BU[NCU][Nf] links U_mu on that backward face
+template <int MU>
+__device__ __forceinline__ int face_index(const Geom& g, const int (&l)[4]) {
+  const int l0h = l[0] >> 1;
+  if (MU == 0) return (l[1] >> 1) + ((l[2] + (l[3] << g.lb[2])) << (g.lb[1] - 1));
+  if (MU == 1) return l0h + ((l[2] + (l[3] << g.lb[2])) << g.lb[0]);
+  if (MU == 2) return l0h + ((l[1] + (l[3] << g.lb[1])) << g.lb[0]);
+  return l0h + ((l[1] + (l[2] << g.lb[1])) << g.lb[0]);
+}
+// inverse: tile-local checkerboard index j of the face site (parity P, face index fidx, l_mu = lmu)
+__device__ __forceinline__ int face_site(const Geom& g, const int mu, const int P, int fidx, const int lmu) {
+  int l[4];
+  if (mu == 0) {
+    const int h1 = g.b[1] >> 1;
+    const int l1h = fidx & (h1 - 1);
+    fidx >>= (g.lb[1] - 1);
+    l[2] = fidx & (g.b[2] - 1);
+    l[3] = fidx >> g.lb[2];
+    l[0] = lmu;
+    l[1] = 2 * l1h + ((P + l[2] + l[3] + lmu) & 1);
+  } else {
+    const int l0h = fidx & ((g.b[0] >> 1) - 1);
+    fidx >>= g.lb[0];
+    const int da = (mu == 1) ? 2 : 1, db = (mu == 3) ? 2 : 3;
+    l[da] = fidx & (g.b[da] - 1);
+    l[db] = fidx >> g.lb[da];
+    l[mu] = lmu;
+    l[0] = 2 * l0h + ((P + l[1] + l[2] + l[3]) & 1);
+  }
+  return local_index(g, l);
+}
+
+// both hops of direction MU for one site: links of the tile in ring stage `ub`, spinor tile `sp`, halo buffer `hb`
 template <typename T, int RECON, int MU>
 __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, const T2<T>* sp, const T2<T>* ub,
-                                         const int* __restrict__ tab, const int tile, const int p, const int j,
-                                         const int (&l)[4], const int x3, const bool nonper, const T sg,
-                                         cx<T> (&acc)[12]) {
+                                         const T2<T>* hb, const int p, const int j, const int (&l)[4], const int x3,
+                                         const bool nonper, const T sg, cx<T> (&acc)[12]) {
   constexpr int NCU = (RECON == 12) ? 6 : 9;
   const int TV = g.TV;
   const int q = 1 - p;
   const int bh0 = g.b[0] >> 1;
   const int l0h = l[0] >> 1;
+  const int Nh = TV >> (MU == 0 ? g.lb[0] + 1 : g.lb[MU]);   // face sites of one parity
+  const int Nf = 2 * Nh;
+  const int fq = q * Nh + face_index<MU>(g, l);
   int stride = bh0;                       // index stride of direction MU (MU >= 1)
   if (MU >= 2) stride <<= g.lb[1];
   if (MU >= 3) stride <<= g.lb[2];
@@ -393,60 +448,91 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
   {
     const bool cr = (l[MU] + 1 == g.b[MU]);
     int jn;
-    if (MU == 0) jn = j - l0h + (cr ? 0 : ((l[0] + 1) >> 1));
-    else jn = cr ? j - (g.b[MU] - 1) * stride : j + stride;
+    if (MU == 0) jn = j - l0h + ((l[0] + 1) >> 1);
+    else jn = j + stride;
     bool on = true;
     if (MU == 3 && nonper) on = !frozen_slice(g, (x3 + 1 == g.L[3]) ? 0 : x3 + 1);
     if (on) {
-      const T2<T>* ps = cr ? a.in + field_offset(g, 12, q, __ldg(tab + 2 * MU), 0, jn) : sp + (size_t)(q * 12) * TV + jn;
-      hop_dir<T, RECON, MU, true, false>(ps, ub + (size_t)(p * NCU) * TV + j, TV, sg, a.has_theta, a.theta[MU], acc);
+      const T2<T>* ps = cr ? hb + fq : sp + (q * 12) * TV + jn;
+      hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, cr ? Nf : TV, TV, sg, a.has_theta, a.theta[MU], acc);
     }
   }
   // ---- backward: theta^* (1 + gamma_mu) U_mu(x - mu)^+ psi(x - mu)
   {
     const bool cr = (l[MU] == 0);
     int jn;
-    if (MU == 0) jn = j - l0h + (cr ? bh0 - 1 : ((l[0] - 1) >> 1));
-    else jn = cr ? j + (g.b[MU] - 1) * stride : j - stride;
+    if (MU == 0) jn = j - l0h + ((l[0] - 1) >> 1);
+    else jn = j - stride;
     bool on = true;
     if (MU == 3 && nonper) on = !frozen_slice(g, (x3 == 0) ? g.L[3] - 1 : x3 - 1);
     if (on) {
-      const T2<T>* ps;
-      const T2<T>* us;
-      if (cr) {
-        const int tn = __ldg(tab + 2 * MU + 1);
-        ps = a.in + field_offset(g, 12, q, tn, 0, jn);
-        us = a.U + field_offset(g, 4 * NCU, q, tn, MU * NCU, jn);
-      } else {
-        ps = sp + (size_t)(q * 12) * TV + jn;
-        us = ub + (size_t)(q * NCU) * TV + jn;
-      }
-      hop_dir<T, RECON, MU, false, false>(ps, us, TV, -sg, a.has_theta, a.theta[MU], acc);
+      const T2<T>* ps = cr ? hb + 12 * Nf + fq : sp + (q * 12) * TV + jn;
+      const T2<T>* us = cr ? hb + 24 * Nf + fq : ub + (q * NCU) * TV + jn;
+      const int sd = cr ? Nf : TV;
+      hop_dir<T, RECON, MU, false, false>(ps, us, sd, sd, -sg, a.has_theta, a.theta[MU], acc);
+    }
+  }
+}
+
+template <typename T> __device__ __forceinline__ void cp_async_elem(T2<T>* dst, const T2<T>* src);
+template <> __device__ __forceinline__ void cp_async_elem<double>(double2* dst, const double2* src) { cp_async_16(dst, src); }
+template <> __device__ __forceinline__ void cp_async_elem<float>(float2* dst, const float2* src) { cp_async_8(dst, src); }
+
+// halo of direction mu of the tile whose table row is `tab` -> buffer hb (layout above); lt = index of this
+// loader thread.
+template <typename T, int NCU>
+__device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, const int* __restrict__ tab, const int mu,
+                                          T2<T>* hb, const int lt) {
+  const int TV = g.TV;
+  const int Nh = TV >> (mu == 0 ? g.lb[0] + 1 : g.lb[mu]);
+  const int Nf = 2 * Nh;
+  const int tf = __ldg(tab + 2 * mu), tb = __ldg(tab + 2 * mu + 1);
+  for (int u = lt; u < 3 * Nf; u += PIPE_HALO_THREADS) {
+    const int kind = u / Nf;           // 0: F, 1: B, 2: BU
+    const int f = u - kind * Nf;       // column: parity-major
+    const int P = f >= Nh ? 1 : 0;
+    const int jn = face_site(g, mu, P, f - P * Nh, kind == 0 ? 0 : g.b[mu] - 1);
+    if (kind < 2) {
+      const T2<T>* src = a.in + field_offset(g, 12, P, kind == 0 ? tf : tb, 0, jn);
+      T2<T>* dst = hb + kind * 12 * Nf + f;
+#pragma unroll
+      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * Nf, src + c * TV);
+    } else {
+      const T2<T>* src = a.U + field_offset(g, 4 * NCU, P, tb, mu * NCU, jn);
+      T2<T>* dst = hb + 24 * Nf + f;
+#pragma unroll
+      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * Nf, src + c * TV);
     }
   }
 }
 
 template <typename T, int RECON, int DIAG>
-__global__ void __launch_bounds__(288, (sizeof(T) == 4) ? 2 : 1)
-dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
+__global__ void __launch_bounds__(PIPE_THREADS, 1)
+dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_elems) {
+  constexpr int nhb = 2;   // halo buffers
   constexpr int NCU = (RECON == 12) ? 6 : 9;
   constexpr int NSTC = (DIAG == DIAG_PRE) ? 36 / NCU : 0;   // clover stages per tile
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ double s_red[9];
+  __shared__ double s_red[PIPE_THREADS / 32];
   if (a.skip != nullptr && *a.skip != 0) return;  // CG finished: uniform early exit
   const int TV = g.TV;
   const int tid = threadIdx.x;
   const int lane = tid & 31;
-  const int ncons = 2 * TV;                         // consumer threads (multiple of 32)
+  const int warp = tid >> 5;
   T2<T>* sp = reinterpret_cast<T2<T>*>(smem_raw);   // [2][12][TV] spinor tile
-  T2<T>* ring = sp + (size_t)24 * TV;               // nslot x [2][NCU][TV]
-  PipeBars* bars = reinterpret_cast<PipeBars*>(ring + (size_t)nslot * 2 * NCU * TV);
+  T2<T>* ring = sp + 24 * TV;                       // nslot x [2][NCU][TV]
+  T2<T>* halo = ring + nslot * 2 * NCU * TV;        // nhb x halo_elems
+  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + nhb * halo_elems);
   if (tid == 0) {
     mbar_init(&bars->full_sp, 1);
-    mbar_init(&bars->empty_sp, ncons >> 5);
+    mbar_init(&bars->empty_sp, PIPE_CONS_WARPS);
+    for (int i = 0; i < nhb; i++) {
+      mbar_init(&bars->full_h[i], PIPE_HALO_THREADS);
+      mbar_init(&bars->empty_h[i], PIPE_CONS_WARPS);
+    }
     for (int i = 0; i < nslot; i++) {
       mbar_init(&bars->full[i], 1);
-      mbar_init(&bars->empty[i], ncons >> 5);
+      mbar_init(&bars->empty[i], PIPE_CONS_WARPS);
     }
     mbar_fence_init();
   }
@@ -455,44 +541,67 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   const uint32_t stage_bytes = (uint32_t)(NCU * TV * sizeof(T2<T>));
   const uint32_t sp_bytes = (uint32_t)(12 * TV * sizeof(T2<T>));
 
-  if (tid >= ncons) {
-    // ------------------------------ producer: one lane feeds the ring ------------------------------
-    if (tid == ncons) {
-      const uint64_t pol_once = policy_evict_first();
-      RingPos rp = {0, 0u};
-      int k = 0;
-      for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x, k++) {
-        if (k == 0) {
-          mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
-          for (int p = 0; p < 2; p++)
-            bulk_g2s(sp + (size_t)(p * 12) * TV, a.in + field_offset(g, 12, p, tile, 0, 0), sp_bytes, &bars->full_sp);
-        }
-#pragma unroll 1
-        for (int st = 0; st < 4 + NSTC; st++) {
-          mbar_wait(&bars->empty[rp.slot], rp.ph ^ 1u);
-          mbar_arrive_expect_tx(&bars->full[rp.slot], 2 * stage_bytes);
-          T2<T>* dst = ring + (size_t)rp.slot * 2 * NCU * TV;
-          for (int p = 0; p < 2; p++) {
-            if (st < 4)
-              bulk_g2s(dst + (size_t)(p * NCU) * TV, a.U + field_offset(g, 4 * NCU, p, tile, st * NCU, 0), stage_bytes,
-                       &bars->full[rp.slot]);
-            else
-              bulk_g2s_hint(dst + (size_t)(p * NCU) * TV, a.A + field_offset(g, 36, p, tile, (st - 4) * NCU, 0),
-                            stage_bytes, &bars->full[rp.slot], pol_once);
+  if (warp >= PIPE_CONS_WARPS) {
+    setmaxnreg_dec<56>();
+    if (warp == PIPE_CONS_WARPS) {
+      // ------------------------------ producer: one lane feeds the ring ------------------------------
+      if (lane == 0) {
+        const uint64_t pol_once = policy_evict_first();
+        RingPos rp = {0, 0u};
+        int k = 0;
+        for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x, k++) {
+          if (k == 0) {
+            mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
+            for (int p = 0; p < 2; p++)
+              bulk_g2s(sp + (p * 12) * TV, a.in + field_offset(g, 12, p, tile, 0, 0), sp_bytes, &bars->full_sp);
           }
-          rp.advance(nslot);
+#pragma unroll 1
+          for (int st = 0; st < 4 + NSTC; st++) {   // stage order: L0 L1 [A+] L2 L3 [A-]  (consumer loop below)
+            constexpr int H = NSTC / 2;
+            int mu = -1, cs = -1;
+            if (st < 2) mu = st;
+            else if (st < 2 + H) cs = st - 2;
+            else if (st < 4 + H) mu = st - H;
+            else cs = st - 4;
+            mbar_wait(&bars->empty[rp.slot], rp.ph ^ 1u);
+            mbar_arrive_expect_tx(&bars->full[rp.slot], 2 * stage_bytes);
+            T2<T>* dst = ring + rp.slot * 2 * NCU * TV;
+            for (int p = 0; p < 2; p++) {
+              if (mu >= 0)
+                bulk_g2s(dst + (p * NCU) * TV, a.U + field_offset(g, 4 * NCU, p, tile, mu * NCU, 0), stage_bytes,
+                         &bars->full[rp.slot]);
+              else   // clover blocks are read exactly once: evict-first keeps them from displacing spinors and links in L2
+                bulk_g2s_hint(dst + (p * NCU) * TV, a.A + field_offset(g, 36, p, tile, cs * NCU, 0), stage_bytes,
+                              &bars->full[rp.slot], pol_once);
+            }
+            rp.advance(nslot);
+          }
+          const int next = tile + gridDim.x;
+          if (next < g.ntiles) {  // spinor of the next tile: its buffer is released after this tile's hops
+            mbar_wait(&bars->empty_sp, (uint32_t)(k & 1));
+            mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
+            for (int p = 0; p < 2; p++)
+              bulk_g2s(sp + (p * 12) * TV, a.in + field_offset(g, 12, p, next, 0, 0), sp_bytes, &bars->full_sp);
+          }
         }
-        const int next = tile + gridDim.x;
-        if (next < g.ntiles) {  // spinor of the next tile: its buffer is released after this tile's hops
-          mbar_wait(&bars->empty_sp, (uint32_t)(k & 1));
-          mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
-          for (int p = 0; p < 2; p++)
-            bulk_g2s(sp + (size_t)(p * 12) * TV, a.in + field_offset(g, 12, p, next, 0, 0), sp_bytes, &bars->full_sp);
+      }
+    } else {
+      // ------------------------------ halo loaders: LDGSTS one stage ahead ----------------------------
+      const int lt = tid - (PIPE_CONS_WARPS + 1) * 32;
+      RingPos hp = {0, 0u};   // halo buffer ring
+      for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x) {
+        const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
+        for (int mu = 0; mu < 4; mu++) {
+          mbar_wait(&bars->empty_h[hp.slot], hp.ph ^ 1u);
+          halo_load<T, NCU>(g, a, tab, mu, halo + hp.slot * halo_elems, lt);
+          cp_async_arrive_noinc(&bars->full_h[hp.slot]);
+          hp.advance(nhb);
         }
       }
     }
   } else {
     // ------------------------------ consumers: one thread per site ---------------------------------
+    setmaxnreg_inc<216>();
     const int p = (tid >= TV) ? 1 : 0;
     const int j = tid - p * TV;
     int l[4];
@@ -500,6 +609,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     const bool nonper = (g.bc != LQCD_BC_PERIODIC);
     const T sg = a.dagger ? T(-1) : T(1);
     RingPos rp = {0, 0u};
+    RingPos hp = {0, 0u};
     int k = 0;
     for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x, k++) {
       const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
@@ -510,33 +620,64 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
       mbar_wait(&bars->full_sp, (uint32_t)(k & 1));
 #define LQCD_HOP_STAGE(MU)                                                                                       \
-      mbar_wait(&bars->full[rp.slot], rp.ph);                                                                    \
-      if (live)                                                                                                  \
-        hop_pair<T, RECON, MU>(g, a, sp, ring + (size_t)rp.slot * 2 * NCU * TV, tab, tile, p, j, l, x3, nonper, sg, acc); \
-      __syncwarp();                                                                                              \
-      if (lane == 0) mbar_arrive(&bars->empty[rp.slot]);                                                         \
-      rp.advance(nslot);
+      {                                                                                                          \
+        const int b = hp.slot;                                                                                   \
+        mbar_wait(&bars->full_h[b], hp.ph);                                                                      \
+        mbar_wait(&bars->full[rp.slot], rp.ph);                                                                  \
+        if (live)                                                                                                \
+          hop_pair<T, RECON, MU>(g, a, sp, ring + rp.slot * 2 * NCU * TV, halo + b * halo_elems, p, j, l, x3,   \
+                                 nonper, sg, acc);                                                               \
+        __syncwarp();                                                                                            \
+        if (lane == 0) {                                                                                         \
+          mbar_arrive(&bars->empty[rp.slot]);                                                                    \
+          mbar_arrive(&bars->empty_h[b]);                                                                        \
+        }                                                                                                        \
+        rp.advance(nslot);                                                                                       \
+        hp.advance(nhb);                                                                                         \
+      }
+      // Stage order H0 H1 [A+ stages] H2 H3 [A- stages]: with two halo buffers every halo then has three stages
+      // of lead.  With the clover term ONE accumulator serves both: acc = sum of hops - (1/k) A psi, result = -k acc,
+      // so that no second 12-component register set is live during the hops.
+      const T2<T>* sv = sp + (p * 12) * TV + j;
       LQCD_HOP_STAGE(0)
       LQCD_HOP_STAGE(1)
+      if (DIAG == DIAG_PRE) {
+        const T s = T(-1) / a.k;
+        if (live) {
+#pragma unroll
+          for (int c = 0; c < 6; c++) {
+            T2<T> w = sv[c * TV];
+            v[c] = cx<T>(s * w.x, s * w.y);
+          }
+        }
+        CloverPipe<T, NCU, 0, NSTC / 2>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
+      }
       LQCD_HOP_STAGE(2)
       LQCD_HOP_STAGE(3)
 #undef LQCD_HOP_STAGE
       if (live) {
-        const T2<T>* sv = sp + (size_t)(p * 12) * TV + j;
+        if (DIAG == DIAG_PRE) {
+          const T s = T(-1) / a.k;
 #pragma unroll
-        for (int c = 0; c < 12; c++) {
-          T2<T> w = sv[c * TV];
-          v[c] = cx<T>(w.x, w.y);
+          for (int c = 6; c < 12; c++) {
+            T2<T> w = sv[c * TV];
+            v[c] = cx<T>(s * w.x, s * w.y);
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 12; c++) {
+            T2<T> w = sv[c * TV];
+            v[c] = cx<T>(w.x, w.y);
+          }
         }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->empty_sp);   // spinor tile no longer needed: next tile's may land
       if (DIAG == DIAG_PRE) {
-        cx<T> av[12];
-        CloverPipe<T, NCU, 0, NSTC>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, av);
+        CloverPipe<T, NCU, NSTC / 2, NSTC>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
         if (live) {
 #pragma unroll
-          for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, av[c].re), fma(-a.k, acc[c].im, av[c].im));
+          for (int c = 0; c < 12; c++) res[c] = cx<T>(-a.k * acc[c].re, -a.k * acc[c].im);
         }
       } else if (live) {
 #pragma unroll
@@ -572,45 +713,64 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   if (a.epi != EPI_STORE) {  // fixed-order CTA reduction over everything this CTA produced
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
-    if (lane == 0) s_red[tid >> 5] = nrm;
+    if (lane == 0) s_red[warp] = nrm;
     __syncthreads();
     if (tid == 0) {
       double s = 0;
-      const int nw = (int)(blockDim.x >> 5);
-      for (int w = 0; w < nw; w++) s += s_red[w];
+      for (int w = 0; w < PIPE_CONS_WARPS; w++) s += s_red[w];
       a.partial[blockIdx.x] = s;
     }
   }
 }
 
+// LQCD_DW_MODE selects the kernel of the full-lattice operator: stream = persistent one-thread-per-site CTAs;
+// split = the same with one parity of a tile per 128-thread CTA; direct = one CTA per tile (hardware scheduling);
+// pipe = the warp-specialised shared-memory pipeline where it applies.
+enum { MODE_STREAM = 0, MODE_DIRECT = 1, MODE_PIPE = 2, MODE_SPLIT = 3 };
+static int dw_mode() {
+  static int mode = -1;
+  if (mode < 0) {
+    const char* e = getenv("LQCD_DW_MODE");
+    mode = MODE_PIPE;   // the pipeline where it applies (full lattice, 128-site tiles), else persistent one-thread-per-site
+    if (e && !strcmp(e, "stream")) mode = MODE_STREAM;
+    if (e && !strcmp(e, "direct")) mode = MODE_DIRECT;
+    if (e && !strcmp(e, "pipe")) mode = MODE_PIPE;
+    if (e && !strcmp(e, "split")) mode = MODE_SPLIT;
+  }
+  return mode;
+}
+static int env_int(const char* name, int dflt) {
+  const char* e = getenv(name);
+  return e ? atoi(e) : dflt;
+}
 // ---- host side: configuration of the persistent kernel ------------------------------------------------
 struct PipeCfg {
   bool use;
-  int grid, threads, nslot;
+  int grid, nslot, halo_elems;
   size_t smem;
 };
 template <typename T>
 static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
   PipeCfg c = {false, 0, 0, 0, 0};
-  static const bool disabled = getenv("LQCD_NO_PIPE") != nullptr;
-  if (disabled || parity >= 0 || diag == DIAG_POST) return c;
-  if (g.TV < 32 || g.TV > 128 || (g.TV & 15) || g.tile_tab == nullptr) return c;
+  if (dw_mode() != MODE_PIPE || parity >= 0 || diag == DIAG_POST) return c;
+  if (g.TV != 128 || g.tile_tab == nullptr) return c;   // 8 consumer warps = both parities of one tile
   const int ncu = recon == 12 ? 6 : 9;
-  const int per_sm = sizeof(T) == 4 ? 2 : 1;
+  int nf = 0;
+  for (int mu = 0; mu < 4; mu++) nf = (2 * g.TV / g.b[mu] > nf) ? 2 * g.TV / g.b[mu] : nf;
+  c.halo_elems = (24 + ncu) * nf;
   const size_t sp = (size_t)24 * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
-  size_t budget = (size_t)g.smem_optin - 256;                            // 256 B: the kernel's static shared memory
-  if (per_sm == 2) budget = ((size_t)g.smem_optin + 1024) / 2 - 1024 - 256;   // 1 KB per CTA is reserved by the system
-  if (budget < sp + sizeof(PipeBars) + 3 * slot) return c;
-  int nslot = (int)((budget - sp - sizeof(PipeBars)) / slot);
-  if (nslot > 8) nslot = 8;
-  const char* e = getenv("LQCD_NSLOT");
-  if (e && atoi(e) >= 2 && atoi(e) <= nslot) nslot = atoi(e);
+  const size_t halo = (size_t)2 * c.halo_elems * sizeof(T2<T>);
+  const size_t budget = (size_t)g.smem_optin - 256;   // 256 B: the kernel's static shared memory
+  if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
+  int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
+  if (nslot > 4) nslot = 4;   // measured: a deeper ring only lets the stream run further ahead of the halos (fp32)
+  const int e = env_int("LQCD_NSLOT", nslot);
+  if (e >= 2 && e <= nslot) nslot = e;
   c.use = true;
   c.nslot = nslot;
-  c.smem = sp + (size_t)nslot * slot + sizeof(PipeBars);
-  c.threads = 2 * g.TV + 32;
-  c.grid = g.sm_count * per_sm;
+  c.smem = sp + (size_t)nslot * slot + halo + sizeof(PipeBars);
+  c.grid = g.sm_count;
   if (c.grid > g.ntiles) c.grid = g.ntiles;
   return c;
 }
@@ -624,15 +784,60 @@ static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg&
     if (e != cudaSuccess) return e;
     attr_smem = c.smem;
   }
-  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, c.threads, c.smem, s>>>(g, a, c.nslot);
+  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, a, c.nslot, c.halo_elems);
   count_launch();
   return cudaGetLastError();
+}
+
+// ---- host side: configuration of the one-thread-per-site kernel ------------------------------------------
+enum { KIND_FULL = 0, KIND_HALF = 1, KIND_SPLIT = 2 };   // dw_kernel / dw_kernel_h<false> / dw_kernel_h<true>
+struct DirectCfg {
+  int grid, threads, kind;
+};
+template <typename T, int RECON, int DIAG>
+static DirectCfg direct_config_t(const Geom& g, int parity) {
+  DirectCfg c;
+  const int mode = dw_mode();
+  const int npar = parity < 0 ? 2 : 1;
+  c.kind = KIND_FULL;
+  if (parity < 0 && mode == MODE_SPLIT) c.kind = KIND_SPLIT;
+  else if (npar * g.TV <= 128 && env_int("LQCD_HALF3", 1)) c.kind = KIND_HALF;
+  c.threads = c.kind == KIND_SPLIT ? ((g.TV + 31) / 32) * 32 : ((npar * g.TV + 31) / 32) * 32;
+  const int items = c.kind == KIND_SPLIT ? 2 * g.ntiles : g.ntiles;
+  c.grid = items;
+  if (mode == MODE_DIRECT) return c;
+  static int per_sm[3] = {0, 0, 0};   // resident CTAs per SM of this instantiation, by kernel kind
+  int& occ = per_sm[c.kind];
+  if (occ == 0) {
+    cudaError_t e;
+    if (c.kind == KIND_FULL) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel<T, RECON, DIAG>, c.threads, 0);
+    else if (c.kind == KIND_HALF) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel_h<T, RECON, DIAG, false>, c.threads, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel_h<T, RECON, DIAG, true>, c.threads, 0);
+    if (e != cudaSuccess || occ < 1) occ = 1;
+  }
+  int ctas = env_int("LQCD_CTAS_PER_SM", occ);
+  if (ctas < 1 || ctas > occ) ctas = occ;
+  c.grid = g.sm_count * ctas;
+  if (c.grid > items) c.grid = items;
+  if (c.kind == KIND_SPLIT) c.grid &= ~1;   // both parities of a tile sit in neighbouring CTAs
+  return c;
+}
+template <typename T>
+static DirectCfg direct_config(const Geom& g, int recon, int diag, int parity) {
+  if (recon == 12) {
+    if (diag == DIAG_ONE) return direct_config_t<T, 12, DIAG_ONE>(g, parity);
+    if (diag == DIAG_PRE) return direct_config_t<T, 12, DIAG_PRE>(g, parity);
+    return direct_config_t<T, 12, DIAG_POST>(g, parity);
+  }
+  if (diag == DIAG_ONE) return direct_config_t<T, 18, DIAG_ONE>(g, parity);
+  if (diag == DIAG_PRE) return direct_config_t<T, 18, DIAG_PRE>(g, parity);
+  return direct_config_t<T, 18, DIAG_POST>(g, parity);
 }
 
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity) {
   PipeCfg c = pipe_config<T>(g, recon, diag, parity);
-  return c.use ? c.grid : g.ntiles;
+  return c.use ? c.grid : direct_config<T>(g, recon, diag, parity).grid;
 }
 template int dw_num_partials<double>(const Geom&, int, int, int);
 template int dw_num_partials<float>(const Geom&, int, int, int);
@@ -678,9 +883,10 @@ template cudaError_t launch_diag<float>(const Geom&, const void*, const void*, v
 
 template <typename T, int RECON, int DIAG>
 static cudaError_t launch_one(const Geom& g, const DwArgs<T>& a, cudaStream_t s) {
-  int npar = a.parity < 0 ? 2 : 1;
-  int threads = ((npar * g.TV + 31) / 32) * 32;
-  dw_kernel<T, RECON, DIAG><<<g.ntiles, threads, 0, s>>>(g, a);
+  const DirectCfg c = direct_config_t<T, RECON, DIAG>(g, a.parity);
+  if (c.kind == KIND_FULL) dw_kernel<T, RECON, DIAG><<<c.grid, c.threads, 0, s>>>(g, a);
+  else if (c.kind == KIND_HALF) dw_kernel_h<T, RECON, DIAG, false><<<c.grid, c.threads, 0, s>>>(g, a);
+  else dw_kernel_h<T, RECON, DIAG, true><<<c.grid, c.threads, 0, s>>>(g, a);
   count_launch();
   return cudaGetLastError();
 }
