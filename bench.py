@@ -247,7 +247,9 @@ def run_ours(args):
     bytes_launch = REALS_DW[recon] * rb * V
     ms_launch = ms_local / launches
     achieved = bytes_launch / (ms_launch * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "dw_kernel", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+    plan = B.dw_plan(S.g, prec, recon, True)
+    roofline = {"bound": "hbm", "kernel": plan.split("<")[0], "launch": plan, "achieved": round(achieved, 1), "peak": peak,
+                "unit": "GB/s",
                 "frac": round(achieved / peak, 4), "peak_source": peak_src,
                 "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
                 "bytes_per_launch": bytes_launch, "ms_per_launch": round(ms_launch, 4),
@@ -282,9 +284,10 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of dw_kernel from the committed ncu --set full
-# capture (profiles/); keyed by (lattice, prec, recon).  None = not captured for that configuration.
-NCU_TRAFFIC = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the stencil kernel from the committed ncu --set full
+# capture (profiles/r01_v2_dw_pipe_kernel_f64_full.txt); keyed by (lattice, prec, recon).  None = not captured for
+# that configuration.
+NCU_TRAFFIC = {("48x48x48x96", "f64", 18): 16760619000 + 2028847000}
 
 
 def run_e2e(torch, B, S, args, L, prec, recon, dist):

@@ -138,6 +138,19 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
                                const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
                                lqcd_recon recon);
 
+/* Which kernel lqcd_dw_apply / lqcd_dwdag_apply (parity = -1) or one half-lattice pass of lqcd_dw_eo_apply
+ * (parity = 0/1) launches for this geometry, precision, link format and clover flag, with its launch
+ * configuration, written as one line of text into buf (at most len bytes, always terminated).  Host only;
+ * for bench.py and the tests.  The choice follows the option "dw_mode" (below) and the tile shape. */
+lqcd_status lqcd_dw_plan(const lqcd_geom* g, lqcd_prec prec, lqcd_recon recon, int has_clover, int parity,
+                         char* buf, int len);
+/* Process-wide options (host strings).  "dw_mode": which stencil kernel serves the full-lattice operator --
+ * "pipe" (default: the warp-specialised shared-memory pipeline where the tile shape allows it), "stream"
+ * (persistent one-thread-per-site CTAs), "split" (one parity of a tile per CTA), "direct" (one CTA per tile).
+ * All four compute the same operator; the environment variable LQCD_DW_MODE sets the initial value.
+ * LQCD_EINVAL for an unknown key or value. */
+lqcd_status lqcd_set_option(const char* key, const char* value);
+
 const char* lqcd_last_error(void);
 /* number of kernels launched by this library since load (for bench.py's gpu_launches) */
 long long lqcd_launch_count(void);

@@ -22,7 +22,8 @@ EXPORTS = [
     "lqcd_gauge_import", "lqcd_gauge_export", "lqcd_spinor_import", "lqcd_spinor_export",
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
-    "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count",
+    "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
+    "lqcd_set_option",
 ]
 
 
@@ -260,3 +261,14 @@ def dw_apply_host(L, kappa, csw, U_canon, psi_canon, out_canon, bc=BC_PERIODIC, 
 
 def launch_count():
     return int(lib().lqcd_launch_count())
+
+
+def dw_plan(g, prec=F64, recon=RECON_18, has_clover=True, parity=-1):
+    """One line naming the stencil kernel and launch configuration lqcd_dw_apply would use."""
+    buf = ctypes.create_string_buffer(512)
+    _check(lib().lqcd_dw_plan(g, prec, recon, 1 if has_clover else 0, parity, buf, 512))
+    return buf.value.decode()
+
+
+def set_option(key, value):
+    _check(lib().lqcd_set_option(key.encode(), value.encode()))

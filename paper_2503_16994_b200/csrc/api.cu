@@ -163,6 +163,27 @@ extern "C" {
 const char* lqcd_last_error(void) { return g_err; }
 long long lqcd_launch_count(void) { return g_launches.load(); }
 
+lqcd_status lqcd_dw_plan(const lqcd_geom* h, lqcd_prec prec, lqcd_recon recon, int has_clover, int parity, char* buf,
+                         int len) {
+  REQUIRE(h && buf && len > 0, "lqcd_dw_plan: NULL argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon) && parity >= -1 && parity <= 1, "lqcd_dw_plan: bad precision, link format or parity");
+  const int diag = has_clover ? DIAG_PRE : DIAG_ONE;
+  const int rc = recon == LQCD_RECON_12 ? 12 : 18;
+  if (prec == LQCD_F64) dw_describe<double>(h->g, rc, diag, parity, buf, len);
+  else dw_describe<float>(h->g, rc, diag, parity, buf, len);
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_set_option(const char* key, const char* value) {
+  REQUIRE(key && value, "lqcd_set_option: NULL argument");
+  if (!strcmp(key, "dw_mode")) {
+    REQUIRE(dw_set_mode(value), "lqcd_set_option: dw_mode must be pipe, stream, split or direct");
+    return LQCD_OK;
+  }
+  set_error("lqcd_set_option: unknown key '%s'", key);
+  return LQCD_EINVAL;
+}
+
 lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   REQUIRE(desc && out, "lqcd_geom_create: NULL argument");
   *out = nullptr;

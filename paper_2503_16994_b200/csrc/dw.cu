@@ -11,6 +11,7 @@
 // out of L1; all loads are 128-bit (fp64) / 64-bit (fp32) and coalesced over the tile-local site index.
 // Epilogues (CG fusion): EPI_STORE, EPI_STORE_NORM (|out|^2 partial per CTA),
 // EPI_AXPY_NORM (r -= alpha*out, |r|^2 partial; out itself is never written).
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -727,17 +728,28 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
 // split = the same with one parity of a tile per 128-thread CTA; direct = one CTA per tile (hardware scheduling);
 // pipe = the warp-specialised shared-memory pipeline where it applies.
 enum { MODE_STREAM = 0, MODE_DIRECT = 1, MODE_PIPE = 2, MODE_SPLIT = 3 };
+static int g_mode = -1;
+static int mode_from_name(const char* e) {
+  if (!e) return -1;
+  if (!strcmp(e, "pipe")) return MODE_PIPE;
+  if (!strcmp(e, "stream")) return MODE_STREAM;
+  if (!strcmp(e, "split")) return MODE_SPLIT;
+  if (!strcmp(e, "direct")) return MODE_DIRECT;
+  return -1;
+}
 static int dw_mode() {
-  static int mode = -1;
-  if (mode < 0) {
-    const char* e = getenv("LQCD_DW_MODE");
-    mode = MODE_PIPE;   // the pipeline where it applies (full lattice, 128-site tiles), else persistent one-thread-per-site
-    if (e && !strcmp(e, "stream")) mode = MODE_STREAM;
-    if (e && !strcmp(e, "direct")) mode = MODE_DIRECT;
-    if (e && !strcmp(e, "pipe")) mode = MODE_PIPE;
-    if (e && !strcmp(e, "split")) mode = MODE_SPLIT;
+  if (g_mode < 0) {
+    g_mode = mode_from_name(getenv("LQCD_DW_MODE"));
+    // default: the pipeline where it applies (full lattice, 128-site tiles), else persistent one-thread-per-site
+    if (g_mode < 0) g_mode = MODE_PIPE;
   }
-  return mode;
+  return g_mode;
+}
+bool dw_set_mode(const char* name) {
+  const int m = mode_from_name(name);
+  if (m < 0) return false;
+  g_mode = m;
+  return true;
 }
 static int env_int(const char* name, int dflt) {
   const char* e = getenv(name);
@@ -833,6 +845,24 @@ static DirectCfg direct_config(const Geom& g, int recon, int diag, int parity) {
   if (diag == DIAG_PRE) return direct_config_t<T, 18, DIAG_PRE>(g, parity);
   return direct_config_t<T, 18, DIAG_POST>(g, parity);
 }
+
+template <typename T>
+void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int len) {
+  const PipeCfg pc = pipe_config<T>(g, recon, diag, parity);
+  const char* tn = sizeof(T) == 8 ? "double" : "float";
+  if (pc.use) {
+    snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=2 tile=%dx%dx%dx%d",
+             tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, g.b[0], g.b[1], g.b[2], g.b[3]);
+    return;
+  }
+  const DirectCfg dc = direct_config<T>(g, recon, diag, parity);
+  snprintf(buf, (size_t)len, "%s<%s,%d,%d%s> grid=%d threads=%d smem=0 tile=%dx%dx%dx%d",
+           dc.kind == KIND_FULL ? "dw_kernel" : "dw_kernel_h", tn, recon, diag,
+           dc.kind == KIND_FULL ? "" : (dc.kind == KIND_SPLIT ? ",split" : ",half"), dc.grid, dc.threads, g.b[0], g.b[1],
+           g.b[2], g.b[3]);
+}
+template void dw_describe<double>(const Geom&, int, int, int, char*, int);
+template void dw_describe<float>(const Geom&, int, int, int, char*, int);
 
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity) {

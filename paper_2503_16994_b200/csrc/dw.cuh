@@ -30,6 +30,11 @@ struct DwArgs {
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity);
 
+// one-line description of the kernel launch_dw would use (lqcd_dw_plan); dw_set_mode: lqcd_set_option("dw_mode")
+template <typename T>
+void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int len);
+bool dw_set_mode(const char* name);
+
 template <typename T>
 cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cudaStream_t s);
 // out(x) = B(x) in(x) on sites of `parity` (-1: all), zero on frozen slices; B = packed 6x6 blocks

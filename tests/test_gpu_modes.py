@@ -1,0 +1,103 @@
+"""-m gpu parity of every stencil-kernel variant ("dw_mode": pipe, stream, split, direct) against the CPU oracle
+on lattices cut into several 4^4 tiles in every direction -- the shape the warp-specialised pipeline kernel
+(dw_pipe_kernel: TMA ring + LDGSTS halo gathers) needs -- for all boundary conditions, both precisions, both link
+formats, D and D^+, with and without the clover term, and through a CG solve (the fused epilogues).
+Tolerances are north_star's (1e-12 fp64, 2e-6 fp32 per-site relative)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2503_16994_b200 import binding as B
+from paper_2503_16994_b200 import synth
+
+from gpu_util import Lattice, interior, round_f32, site_rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL = {B.F64: 1e-12, B.F32: 2e-6}
+MODES = ["pipe", "stream", "split", "direct"]
+KERNEL = {"pipe": "dw_pipe_kernel", "stream": "dw_kernel<", "split": "dw_kernel_h<", "direct": "dw_kernel<"}
+
+# several 4^4 tiles per direction, unequal tile counts, odd tile counts (3 along one axis)
+CASES = [
+    ((8, 8, 8, 8), B.BC_PERIODIC, (0.3, -0.2, 0.1, np.pi), None),
+    ((8, 4, 12, 8), B.BC_OPEN, (0.5, 0.5, 0.5, 0.0), None),
+    ((4, 8, 8, 12), B.BC_SF_ORBI, (0.5, 0.5, 0.5, 0.0), synth.SF_PHIT),
+]
+
+
+@pytest.fixture
+def mode(request):
+    B.set_option("dw_mode", request.param)
+    yield request.param
+    B.set_option("dw_mode", "pipe")
+
+
+def inputs(L, bc, seed):
+    U = synth.smooth_gauge(L, seed)
+    if bc in (B.BC_SF_ORBI, B.BC_SF_AFWB):
+        U = synth.apply_sf_boundary(L, U)
+    return U, synth.gaussian_spinor(L, seed + 1)
+
+
+@pytest.mark.parametrize("mode", MODES, indirect=True)
+@pytest.mark.parametrize("L,bc,theta,phiT", CASES)
+@pytest.mark.parametrize("prec,recon", [(B.F64, B.RECON_18), (B.F64, B.RECON_12), (B.F32, B.RECON_18), (B.F32, B.RECON_12)])
+def test_dw_parity_every_kernel(mode, L, bc, theta, phiT, prec, recon):
+    kappa, csw = 0.137, 1.9
+    U, psi = inputs(L, bc, 61)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc, phiT=phiT)
+    Uo, psio, Ao = (round_f32(U), round_f32(psi), round_f32(A)) if prec == B.F32 else (U, psi, A)
+    lat = Lattice(L, bc, theta, synth.SF_PHI0, phiT)
+    assert B.geom_info(lat.g)[0] == [4, 4, 4, 4]
+    assert KERNEL[mode] in B.dw_plan(lat.g, prec, recon, True)
+    lat.set_gauge(U, recons=(recon,), precs=(prec,))
+    lat.build_clover(kappa, csw, recon=recon, precs=(prec,))
+    mask = interior(L, bc)
+    for dagger in (False, True):
+        ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=bc, theta=theta, dagger=dagger)
+        got = lat.dw(kappa, psi, prec, recon, dagger)
+        assert site_rel_err(got, ref, mask) <= TOL[prec]
+        assert np.all(got[~mask] == 0)
+    ref = oracle.dw(L, Uo, psio, kappa, None, bc=bc, theta=theta)
+    got = lat.dw(kappa, psi, prec, recon, clover=False)
+    assert site_rel_err(got, ref, mask) <= TOL[prec]
+    lat.close()
+
+
+@pytest.mark.parametrize("mode", MODES, indirect=True)
+def test_cg_every_kernel(mode):
+    """The fused epilogues (|Dp|^2 in the D kernel; r -= alpha D^+t and |r|^2 in the D^+ kernel) of each variant:
+    a full CG solve must reach the requested residual and agree with the oracle's solution."""
+    L, kappa, csw = (8, 8, 4, 8), 0.125, 1.0
+    U, b = inputs(L, B.BC_PERIODIC, 71)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    lat = Lattice(L)
+    lat.set_gauge(U)
+    lat.build_clover(kappa, csw)
+    src = lat.spinor(b)
+    x = lat.alloc(B.FIELD_SPINOR)
+    ws = lat.alloc(B.FIELD_WORKSPACE)
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, x, ws, tol=1e-10, maxiter=4000)
+    assert info["status"] == B.OK and info["rel_resid_normal"] <= 1e-10
+    xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, tol=1e-10)
+    got = lat.spinor_to_host(x)
+    assert np.linalg.norm(got - xo) / np.linalg.norm(xo) <= 1e-8
+    assert abs(info["iters"] - it_o) <= 2
+    lat.close()
+
+
+def test_plan_and_option_errors():
+    lat = Lattice((8, 8, 8, 8))
+    assert "dw_pipe_kernel<double,18,1>" in B.dw_plan(lat.g)
+    assert "ring_slots=3" in B.dw_plan(lat.g)                       # fp64: 3 x 36 KB stages + 2 x 33 KB halos + 48 KB tile
+    assert "dw_kernel_h<float,12,1,half>" in B.dw_plan(lat.g, B.F32, B.RECON_12, True, parity=1)   # half-lattice pass
+    with pytest.raises(B.LqcdError):
+        B.set_option("dw_mode", "bogus")
+    with pytest.raises(B.LqcdError):
+        B.set_option("nonsense", "1")
+    lat.close()
+    small = Lattice((12, 6, 10, 8))    # extents not divisible by 4: no 4^4 tiles, the pipeline does not apply
+    assert "dw_pipe_kernel" not in B.dw_plan(small.g)
+    small.close()
