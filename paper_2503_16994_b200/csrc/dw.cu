@@ -356,7 +356,11 @@ struct CloverStage<T, C0, 0> {
   static __device__ __forceinline__ void run(const T2<T>*, const int, const cx<T> (&)[12], cx<T> (&)[12]) {}
 };
 
-enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12 };
+// The pipeline kernel is written for 4x4x4x4 tiles: TV = 128 sites of one parity, every face 2*TV/4 = 64 columns.
+// With both fixed at compile time every shared-memory access of the arithmetic warps is an immediate offset from
+// one base register, and the two halo buffers interleave into rows of 2*PIPE_NF = PIPE_TV columns, i.e. halo rows
+// have the same stride as tile rows and a hop needs no stride select.
+enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12, PIPE_TV = 128, PIPE_NF = 64 };
 struct PipeBars {
   uint64_t full_sp, empty_sp;
   uint64_t full_h[2], empty_h[2];
@@ -398,35 +402,29 @@ struct CloverPipe<T, NCU, NS, NS> {
 //   F [12][Nf]  spinors of the +mu neighbour tile on its face l_mu = 0        (forward hops leaving the tile)
 //   B [12][Nf]  spinors of the -mu neighbour tile on its face l_mu = b_mu - 1 (backward hops leaving the tile)
 //   BU[NCU][Nf] links U_mu on that backward face
+// stored as rows of PIPE_TV columns: buffer 0 in columns [0, Nf), buffer 1 in columns [Nf, 2 Nf).
 template <int MU>
-__device__ __forceinline__ int face_index(const Geom& g, const int (&l)[4]) {
+__device__ __forceinline__ int face_index(const int (&l)[4]) {   // 4x4x4x4 tile
   const int l0h = l[0] >> 1;
-  if (MU == 0) return (l[1] >> 1) + ((l[2] + (l[3] << g.lb[2])) << (g.lb[1] - 1));
-  if (MU == 1) return l0h + ((l[2] + (l[3] << g.lb[2])) << g.lb[0]);
-  if (MU == 2) return l0h + ((l[1] + (l[3] << g.lb[1])) << g.lb[0]);
-  return l0h + ((l[1] + (l[2] << g.lb[1])) << g.lb[0]);
+  if (MU == 0) return (l[1] >> 1) + 2 * (l[2] + 4 * l[3]);
+  if (MU == 1) return l0h + 2 * (l[2] + 4 * l[3]);
+  if (MU == 2) return l0h + 2 * (l[1] + 4 * l[3]);
+  return l0h + 2 * (l[1] + 4 * l[2]);
 }
-// inverse: tile-local checkerboard index j of the face site (parity P, face index fidx, l_mu = lmu)
-__device__ __forceinline__ int face_site(const Geom& g, const int mu, const int P, int fidx, const int lmu) {
-  int l[4];
+// inverse: tile-local checkerboard index j of the face site (parity P, face index fidx, l_mu = lmu), 4x4x4x4 tile
+__device__ __forceinline__ int face_site(const int mu, const int P, const int fidx, const int lmu) {
+  const int lo = fidx & 1, mid = (fidx >> 1) & 3, hi = fidx >> 3;
+  int l0, l1, l2, l3;
   if (mu == 0) {
-    const int h1 = g.b[1] >> 1;
-    const int l1h = fidx & (h1 - 1);
-    fidx >>= (g.lb[1] - 1);
-    l[2] = fidx & (g.b[2] - 1);
-    l[3] = fidx >> g.lb[2];
-    l[0] = lmu;
-    l[1] = 2 * l1h + ((P + l[2] + l[3] + lmu) & 1);
+    l2 = mid; l3 = hi; l0 = lmu;
+    l1 = 2 * lo + ((P + l2 + l3 + lmu) & 1);
   } else {
-    const int l0h = fidx & ((g.b[0] >> 1) - 1);
-    fidx >>= g.lb[0];
-    const int da = (mu == 1) ? 2 : 1, db = (mu == 3) ? 2 : 3;
-    l[da] = fidx & (g.b[da] - 1);
-    l[db] = fidx >> g.lb[da];
-    l[mu] = lmu;
-    l[0] = 2 * l0h + ((P + l[1] + l[2] + l[3]) & 1);
+    if (mu == 1) { l1 = lmu; l2 = mid; l3 = hi; }
+    else if (mu == 2) { l1 = mid; l2 = lmu; l3 = hi; }
+    else { l1 = mid; l2 = hi; l3 = lmu; }
+    l0 = 2 * lo + ((P + l1 + l2 + l3) & 1);
   }
-  return local_index(g, l);
+  return (l0 >> 1) + 2 * (l1 + 4 * (l2 + 4 * l3));
 }
 
 // both hops of direction MU for one site: links of the tile in ring stage `ub`, spinor tile `sp`, halo buffer `hb`
@@ -435,19 +433,14 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
                                          const T2<T>* hb, const int p, const int j, const int (&l)[4], const int x3,
                                          const bool nonper, const T sg, cx<T> (&acc)[12]) {
   constexpr int NCU = (RECON == 12) ? 6 : 9;
-  const int TV = g.TV;
+  constexpr int TV = PIPE_TV, Nh = PIPE_NF / 2;
   const int q = 1 - p;
-  const int bh0 = g.b[0] >> 1;
   const int l0h = l[0] >> 1;
-  const int Nh = TV >> (MU == 0 ? g.lb[0] + 1 : g.lb[MU]);   // face sites of one parity
-  const int Nf = 2 * Nh;
-  const int fq = q * Nh + face_index<MU>(g, l);
-  int stride = bh0;                       // index stride of direction MU (MU >= 1)
-  if (MU >= 2) stride <<= g.lb[1];
-  if (MU >= 3) stride <<= g.lb[2];
+  const int fq = q * Nh + face_index<MU>(l);
+  constexpr int stride = MU == 1 ? 2 : (MU == 2 ? 8 : 32);   // index stride of direction MU (MU >= 1)
   // ---- forward: theta (1 - gamma_mu) U_mu(x) psi(x + mu)
   {
-    const bool cr = (l[MU] + 1 == g.b[MU]);
+    const bool cr = (l[MU] == 3);
     int jn;
     if (MU == 0) jn = j - l0h + ((l[0] + 1) >> 1);
     else jn = j + stride;
@@ -455,7 +448,7 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
     if (MU == 3 && nonper) on = !frozen_slice(g, (x3 + 1 == g.L[3]) ? 0 : x3 + 1);
     if (on) {
       const T2<T>* ps = cr ? hb + fq : sp + (q * 12) * TV + jn;
-      hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, cr ? Nf : TV, TV, sg, a.has_theta, a.theta[MU], acc);
+      hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, TV, TV, sg, a.has_theta, a.theta[MU], acc);
     }
   }
   // ---- backward: theta^* (1 + gamma_mu) U_mu(x - mu)^+ psi(x - mu)
@@ -467,10 +460,9 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
     bool on = true;
     if (MU == 3 && nonper) on = !frozen_slice(g, (x3 == 0) ? g.L[3] - 1 : x3 - 1);
     if (on) {
-      const T2<T>* ps = cr ? hb + 12 * Nf + fq : sp + (q * 12) * TV + jn;
-      const T2<T>* us = cr ? hb + 24 * Nf + fq : ub + (q * NCU) * TV + jn;
-      const int sd = cr ? Nf : TV;
-      hop_dir<T, RECON, MU, false, false>(ps, us, sd, sd, -sg, a.has_theta, a.theta[MU], acc);
+      const T2<T>* ps = cr ? hb + 12 * TV + fq : sp + (q * 12) * TV + jn;
+      const T2<T>* us = cr ? hb + 24 * TV + fq : ub + (q * NCU) * TV + jn;
+      hop_dir<T, RECON, MU, false, false>(ps, us, TV, TV, -sg, a.has_theta, a.theta[MU], acc);
     }
   }
 }
@@ -484,46 +476,44 @@ template <> __device__ __forceinline__ void cp_async_elem<float>(float2* dst, co
 template <typename T, int NCU>
 __device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, const int* __restrict__ tab, const int mu,
                                           T2<T>* hb, const int lt) {
-  const int TV = g.TV;
-  const int Nh = TV >> (mu == 0 ? g.lb[0] + 1 : g.lb[mu]);
-  const int Nf = 2 * Nh;
+  constexpr int TV = PIPE_TV, Nf = PIPE_NF, Nh = PIPE_NF / 2;
   const int tf = __ldg(tab + 2 * mu), tb = __ldg(tab + 2 * mu + 1);
   for (int u = lt; u < 3 * Nf; u += PIPE_HALO_THREADS) {
     const int kind = u / Nf;           // 0: F, 1: B, 2: BU
     const int f = u - kind * Nf;       // column: parity-major
     const int P = f >= Nh ? 1 : 0;
-    const int jn = face_site(g, mu, P, f - P * Nh, kind == 0 ? 0 : g.b[mu] - 1);
+    const int jn = face_site(mu, P, f - P * Nh, kind == 0 ? 0 : 3);
     if (kind < 2) {
       const T2<T>* src = a.in + field_offset(g, 12, P, kind == 0 ? tf : tb, 0, jn);
-      T2<T>* dst = hb + kind * 12 * Nf + f;
+      T2<T>* dst = hb + kind * 12 * TV + f;
 #pragma unroll
-      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * Nf, src + c * TV);
+      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * TV, src + c * TV);
     } else {
       const T2<T>* src = a.U + field_offset(g, 4 * NCU, P, tb, mu * NCU, jn);
-      T2<T>* dst = hb + 24 * Nf + f;
+      T2<T>* dst = hb + 24 * TV + f;
 #pragma unroll
-      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * Nf, src + c * TV);
+      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * TV, src + c * TV);
     }
   }
 }
 
 template <typename T, int RECON, int DIAG>
 __global__ void __launch_bounds__(PIPE_THREADS, 1)
-dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_elems) {
-  constexpr int nhb = 2;   // halo buffers
+dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
+  constexpr int nhb = 2;   // halo buffers: columns [0, PIPE_NF) and [PIPE_NF, PIPE_TV) of the halo rows
   constexpr int NCU = (RECON == 12) ? 6 : 9;
   constexpr int NSTC = (DIAG == DIAG_PRE) ? 36 / NCU : 0;   // clover stages per tile
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ double s_red[PIPE_THREADS / 32];
   if (a.skip != nullptr && *a.skip != 0) return;  // CG finished: uniform early exit
-  const int TV = g.TV;
+  constexpr int TV = PIPE_TV;
   const int tid = threadIdx.x;
   const int lane = tid & 31;
   const int warp = tid >> 5;
   T2<T>* sp = reinterpret_cast<T2<T>*>(smem_raw);   // [2][12][TV] spinor tile
   T2<T>* ring = sp + 24 * TV;                       // nslot x [2][NCU][TV]
-  T2<T>* halo = ring + nslot * 2 * NCU * TV;        // nhb x halo_elems
-  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + nhb * halo_elems);
+  T2<T>* halo = ring + nslot * 2 * NCU * TV;        // [24 + NCU][PIPE_TV]: both halo buffers
+  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * TV);
   if (tid == 0) {
     mbar_init(&bars->full_sp, 1);
     mbar_init(&bars->empty_sp, PIPE_CONS_WARPS);
@@ -564,7 +554,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
             else if (st < 2 + H) cs = st - 2;
             else if (st < 4 + H) mu = st - H;
             else cs = st - 4;
-            mbar_wait(&bars->empty[rp.slot], rp.ph ^ 1u);
+            mbar_wait_relaxed(&bars->empty[rp.slot], rp.ph ^ 1u);
             mbar_arrive_expect_tx(&bars->full[rp.slot], 2 * stage_bytes);
             T2<T>* dst = ring + rp.slot * 2 * NCU * TV;
             for (int p = 0; p < 2; p++) {
@@ -579,7 +569,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
           }
           const int next = tile + gridDim.x;
           if (next < g.ntiles) {  // spinor of the next tile: its buffer is released after this tile's hops
-            mbar_wait(&bars->empty_sp, (uint32_t)(k & 1));
+            mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
               bulk_g2s(sp + (p * 12) * TV, a.in + field_offset(g, 12, p, next, 0, 0), sp_bytes, &bars->full_sp);
@@ -593,8 +583,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
       for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x) {
         const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
         for (int mu = 0; mu < 4; mu++) {
-          mbar_wait(&bars->empty_h[hp.slot], hp.ph ^ 1u);
-          halo_load<T, NCU>(g, a, tab, mu, halo + hp.slot * halo_elems, lt);
+          mbar_wait_relaxed(&bars->empty_h[hp.slot], hp.ph ^ 1u);
+          halo_load<T, NCU>(g, a, tab, mu, halo + hp.slot * PIPE_NF, lt);
           cp_async_arrive_noinc(&bars->full_h[hp.slot]);
           hp.advance(nhb);
         }
@@ -605,8 +595,11 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
     setmaxnreg_inc<216>();
     const int p = (tid >= TV) ? 1 : 0;
     const int j = tid - p * TV;
-    int l[4];
-    local_coords(g, j, p, l);
+    int l[4];   // 4x4x4x4 tile: j = l0/2 + 2 (l1 + 4 (l2 + 4 l3))
+    l[1] = (j >> 1) & 3;
+    l[2] = (j >> 3) & 3;
+    l[3] = j >> 5;
+    l[0] = 2 * (j & 1) + ((p + l[1] + l[2] + l[3]) & 1);
     const bool nonper = (g.bc != LQCD_BC_PERIODIC);
     const T sg = a.dagger ? T(-1) : T(1);
     RingPos rp = {0, 0u};
@@ -626,7 +619,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot, const int halo_
         mbar_wait(&bars->full_h[b], hp.ph);                                                                      \
         mbar_wait(&bars->full[rp.slot], rp.ph);                                                                  \
         if (live)                                                                                                \
-          hop_pair<T, RECON, MU>(g, a, sp, ring + rp.slot * 2 * NCU * TV, halo + b * halo_elems, p, j, l, x3,   \
+          hop_pair<T, RECON, MU>(g, a, sp, ring + rp.slot * 2 * NCU * TV, halo + b * PIPE_NF, p, j, l, x3,     \
                                  nonper, sg, acc);                                                               \
         __syncwarp();                                                                                            \
         if (lane == 0) {                                                                                         \
@@ -758,21 +751,18 @@ static int env_int(const char* name, int dflt) {
 // ---- host side: configuration of the persistent kernel ------------------------------------------------
 struct PipeCfg {
   bool use;
-  int grid, nslot, halo_elems;
+  int grid, nslot;
   size_t smem;
 };
 template <typename T>
 static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
-  PipeCfg c = {false, 0, 0, 0, 0};
+  PipeCfg c = {false, 0, 0, 0};
   if (dw_mode() != MODE_PIPE || parity >= 0 || diag == DIAG_POST) return c;
-  if (g.TV != 128 || g.tile_tab == nullptr) return c;   // 8 consumer warps = both parities of one tile
+  if (g.b[0] != 4 || g.b[1] != 4 || g.b[2] != 4 || g.b[3] != 4 || g.tile_tab == nullptr) return c;   // PIPE_TV, PIPE_NF
   const int ncu = recon == 12 ? 6 : 9;
-  int nf = 0;
-  for (int mu = 0; mu < 4; mu++) nf = (2 * g.TV / g.b[mu] > nf) ? 2 * g.TV / g.b[mu] : nf;
-  c.halo_elems = (24 + ncu) * nf;
   const size_t sp = (size_t)24 * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
-  const size_t halo = (size_t)2 * c.halo_elems * sizeof(T2<T>);
+  const size_t halo = (size_t)(24 + ncu) * PIPE_TV * sizeof(T2<T>);   // both buffers
   const size_t budget = (size_t)g.smem_optin - 256;   // 256 B: the kernel's static shared memory
   if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
   int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
@@ -796,7 +786,7 @@ static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg&
     if (e != cudaSuccess) return e;
     attr_smem = c.smem;
   }
-  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, a, c.nslot, c.halo_elems);
+  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, a, c.nslot);
   count_launch();
   return cudaGetLastError();
 }

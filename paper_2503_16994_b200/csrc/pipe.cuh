@@ -35,6 +35,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
+// the same for the producer side, which is normally far ahead and would otherwise spend its time re-issuing the
+// probe: a failed probe sleeps before the next one, leaving the issue slots (and the power) to the arithmetic warps
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  for (;;) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    if (done) break;
+    __nanosleep(128);
+  }
+}
+
 // L2 eviction policies for the bulk copies (data used once vs data re-read by neighbouring tiles)
 __device__ __forceinline__ uint64_t policy_evict_first() {
   uint64_t p;
