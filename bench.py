@@ -167,7 +167,7 @@ class Setup:
             A = B.alloc_field(self.g, B.FIELD_CLOVER, prec)
             Ai = B.alloc_field(self.g, B.FIELD_CLOVER, prec) if inverse else None
             self.clover_ms = time_calls(
-                torch, lambda: B.clover_build(self.g, kappa, csw, self.U[(B.F64, r0)], A, Ai, r0, prec), 1, 0)
+                torch, lambda: B.clover_build(self.g, kappa, csw, self.U[(B.F64, r0)], A, Ai, r0, prec), 1, 1)
             self.A[prec], self.Ainv[prec] = A, Ai
             self.psi[prec] = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
             self.out[prec] = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
