@@ -372,6 +372,21 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
                     "ms": round(ms, 4), "GFLOP/s": round(FLOP_DW * V / ms / 1e6, 1), "GB/s": gbs(REALS_DW[r], rb, ms),
                     "frac_measured_peak": round(gbs(REALS_DW[r], rb, ms) / peak, 4)}
     rows["a4_dw"] = dw
+    # NEXT-1: 12 right-hand sides in one pass (links and clover blocks from HBM once per tile)
+    nrhs = 12
+    fb = B.field_bytes(g, B.FIELD_SPINOR, B.F64)
+    src = torch.empty(nrhs * fb, dtype=torch.uint8, device="cuda")
+    dst = torch.empty_like(src)
+    for n in range(nrhs):
+        src[n * fb:(n + 1) * fb].copy_(S.psi[B.F64])
+    ms = time_calls(torch, lambda: B.dw_apply_multi(g, kappa, S.U[(B.F64, recon)], S.A[B.F64], src, dst, nrhs, B.F64, recon), 3)
+    reals_multi = (REALS_DW[recon] - 48) + 48 * nrhs
+    rows["next1_dw_multi_12rhs_f64"] = {
+        "ms": round(ms, 3), "ms_per_rhs": round(ms / nrhs, 4), "GFLOP/s": round(nrhs * FLOP_DW * V / ms / 1e6, 1),
+        "GB/s_model": gbs(reals_multi, 8, ms), "model": "%d reals/site for 12 columns (links + clover once)" % reals_multi,
+        "note": "no gain over 12 single applications yet: with the links served by L2 the pipeline is bound by its "
+                "arithmetic warps (about 2.6 ms per right-hand side)"}
+    del src, dst
     # a6: BLAS-1 reduction alone (|v|^2 over one spinor)
     ws = B.alloc_field(g, B.FIELD_WORKSPACE)
     ms = time_calls(torch, lambda: B.spinor_norm2(g, S.psi[B.F64], ws), 10)

@@ -138,6 +138,15 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
                                const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
                                lqcd_recon recon);
 
+/* SURVEY.md 8(f) NEXT-1 (the 12 colour-spin sources of propagator! share one gauge field): D or D^+
+ * (dagger != 0) applied to nrhs (1..64) spinor fields in one pass.  in / out: DEVICE arrays of nrhs internal spinor
+ * fields stored back to back (lqcd_field_bytes(SPINOR) apart), caller-owned, not overlapping.  Links and clover
+ * blocks are fetched from HBM once per tile and serve all right-hand sides (the 2nd..nth come out of L2), i.e.
+ * 144 + 48 nrhs reals per site instead of 192 nrhs.  Same result, bit for bit, as nrhs separate calls. */
+lqcd_status lqcd_dw_apply_multi(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* clover,
+                                const void* in, void* out, int nrhs, int dagger, lqcd_prec prec, lqcd_recon recon,
+                                void* stream);
+
 /* Which kernel lqcd_dw_apply / lqcd_dwdag_apply (parity = -1) or one half-lattice pass of lqcd_dw_eo_apply
  * (parity = 0/1) launches for this geometry, precision, link format and clover flag, with its launch
  * configuration, written as one line of text into buf (at most len bytes, always terminated).  Host only;

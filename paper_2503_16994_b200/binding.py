@@ -23,7 +23,7 @@ EXPORTS = [
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
-    "lqcd_set_option",
+    "lqcd_set_option", "lqcd_dw_apply_multi",
 ]
 
 
@@ -257,6 +257,13 @@ def dw_apply_host(L, kappa, csw, U_canon, psi_canon, out_canon, bc=BC_PERIODIC, 
     d = _dirac(kappa, csw, ct)
     _check(lib().lqcd_dw_apply_host(ctypes.byref(desc), ctypes.byref(d), _ptr(U_canon), _ptr(psi_canon), _ptr(out_canon),
                                     1 if dagger else 0, prec, recon))
+
+
+def dw_apply_multi(g, kappa, U, clover, src, dst, nrhs, prec=F64, recon=RECON_18, dagger=False, stream=None):
+    """D (or D^+) on nrhs spinor fields stored back to back in src / dst."""
+    d = _dirac(kappa)
+    _check(lib().lqcd_dw_apply_multi(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(src), _ptr(dst), int(nrhs),
+                                     1 if dagger else 0, prec, recon, _stream(stream)))
 
 
 def launch_count():

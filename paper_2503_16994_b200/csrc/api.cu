@@ -353,7 +353,29 @@ static cudaError_t dw_apply_t(const lqcd_geom* h, const lqcd_dirac* d, const voi
   return M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s);
 }
 
+template <typename T>
+static cudaError_t dw_multi_t(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                              void* out, int nrhs, bool dagger, int recon, cudaStream_t s) {
+  Op<T> M;
+  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.recon = recon; M.eo = false;
+  return M.apply_multi(in, out, nrhs, dagger, s);
+}
+
 extern "C" {
+lqcd_status lqcd_dw_apply_multi(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                                void* out, int nrhs, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && U && in && out, "lqcd_dw_apply_multi: NULL argument");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply_multi: bad precision / recon");
+  REQUIRE(nrhs >= 1 && nrhs <= 64, "lqcd_dw_apply_multi: nrhs must be in 1..64");
+  const size_t fb = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon);
+  const char *ib = (const char*)in, *ob = (const char*)out;
+  REQUIRE(ob + nrhs * fb <= ib || ib + nrhs * fb <= ob, "lqcd_dw_apply_multi: input and output arrays overlap");
+  REQUIRE(out != U && out != clover, "lqcd_dw_apply_multi: output aliases an input");
+  CUDA_TRY(DISPATCH_PREC(prec, dw_multi_t<double>(h, d, U, clover, in, out, nrhs, dagger != 0, (int)recon, as_stream(stream)),
+                         dw_multi_t<float>(h, d, U, clover, in, out, nrhs, dagger != 0, (int)recon, as_stream(stream))),
+           "dw kernel (multi)");
+  return LQCD_OK;
+}
 static lqcd_status dw_common(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
                              void* out, lqcd_prec prec, lqcd_recon recon, void* stream, bool dagger) {
   REQUIRE(h && d && U && in && out, "lqcd_dw_apply: NULL argument");

@@ -59,6 +59,26 @@ cudaError_t Op<T>::apply(const void* in, void* out, bool dagger, int epi, void* 
   return launch_dw<T>(geom->g, a, recon, DIAG_PRE, s);
 }
 
+template <typename T>
+cudaError_t Op<T>::apply_multi(const void* in, void* out, int nrhs, bool dagger, cudaStream_t s) const {
+  DwArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.U = (const T2<T>*)U;
+  a.A = (const T2<T>*)A;
+  a.in = (const T2<T>*)in;
+  a.self = (const T2<T>*)in;
+  a.out = (T2<T>*)out;
+  a.k = (T)kappa;
+  a.has_theta = geom->has_theta;
+  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  a.dagger = dagger ? 1 : 0;
+  a.parity = -1;
+  a.epi = EPI_STORE;
+  a.nrhs = nrhs;
+  a.rhs_stride = (long long)2 * geom->g.Vh * 12;
+  return launch_dw<T>(geom->g, a, recon, A ? DIAG_PRE : DIAG_ONE, s);
+}
+
 // out(parity) = self - k * H in   (no clover), used by the even-odd source preparation / reconstruction
 template <typename T>
 cudaError_t Op<T>::hop_xpay(const void* in, const void* self, void* out, double k, int parity, cudaStream_t s) const {

@@ -18,6 +18,8 @@ struct Op {
   // out = M in or M^+ in, with the fused epilogue `epi` (dw.cuh)
   cudaError_t apply(const void* in, void* out, bool dagger, int epi, void* r, const double* alpha, double* partial,
                     const int* skip, cudaStream_t s) const;
+  // full operator on nrhs spinor fields stored back to back (in[n], out[n] one full field apart), EPI_STORE
+  cudaError_t apply_multi(const void* in, void* out, int nrhs, bool dagger, cudaStream_t s) const;
   cudaError_t hop_xpay(const void* in, const void* self, void* out, double k, int parity, cudaStream_t s) const;
 };
 

@@ -474,8 +474,8 @@ template <> __device__ __forceinline__ void cp_async_elem<float>(float2* dst, co
 // halo of direction mu of the tile whose table row is `tab` -> buffer hb (layout above); lt = index of this
 // loader thread.
 template <typename T, int NCU>
-__device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, const int* __restrict__ tab, const int mu,
-                                          T2<T>* hb, const int lt) {
+__device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, const T2<T>* __restrict__ in,
+                                          const int* __restrict__ tab, const int mu, T2<T>* hb, const int lt) {
   constexpr int TV = PIPE_TV, Nf = PIPE_NF, Nh = PIPE_NF / 2;
   const int tf = __ldg(tab + 2 * mu), tb = __ldg(tab + 2 * mu + 1);
   for (int u = lt; u < 3 * Nf; u += PIPE_HALO_THREADS) {
@@ -484,7 +484,7 @@ __device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, con
     const int P = f >= Nh ? 1 : 0;
     const int jn = face_site(mu, P, f - P * Nh, kind == 0 ? 0 : 3);
     if (kind < 2) {
-      const T2<T>* src = a.in + field_offset(g, 12, P, kind == 0 ? tf : tb, 0, jn);
+      const T2<T>* src = in + field_offset(g, 12, P, kind == 0 ? tf : tb, 0, jn);
       T2<T>* dst = hb + kind * 12 * TV + f;
 #pragma unroll
       for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * TV, src + c * TV);
@@ -529,6 +529,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   }
   __syncthreads();
   double nrm = 0.0;
+  const int nrhs = a.nrhs > 1 ? a.nrhs : 1;
   const uint32_t stage_bytes = (uint32_t)(NCU * TV * sizeof(T2<T>));
   const uint32_t sp_bytes = (uint32_t)(12 * TV * sizeof(T2<T>));
 
@@ -540,7 +541,9 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         const uint64_t pol_once = policy_evict_first();
         RingPos rp = {0, 0u};
         int k = 0;
-        for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x, k++) {
+        for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+        for (int rhs = 0; rhs < nrhs; rhs++, k++) {   // all right-hand sides of a tile back to back: links and clover
+                                                       // blocks of the 2nd..nth pass come out of L2
           if (k == 0) {
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
@@ -561,18 +564,23 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
               if (mu >= 0)
                 bulk_g2s(dst + (p * NCU) * TV, a.U + field_offset(g, 4 * NCU, p, tile, mu * NCU, 0), stage_bytes,
                          &bars->full[rp.slot]);
-              else   // clover blocks are read exactly once: evict-first keeps them from displacing spinors and links in L2
+              else if (rhs + 1 < nrhs)
+                bulk_g2s(dst + (p * NCU) * TV, a.A + field_offset(g, 36, p, tile, cs * NCU, 0), stage_bytes,
+                         &bars->full[rp.slot]);
+              else   // clover blocks are read for the last time: evict-first keeps them from displacing spinors and links in L2
                 bulk_g2s_hint(dst + (p * NCU) * TV, a.A + field_offset(g, 36, p, tile, cs * NCU, 0), stage_bytes,
                               &bars->full[rp.slot], pol_once);
             }
             rp.advance(nslot);
           }
-          const int next = tile + gridDim.x;
-          if (next < g.ntiles) {  // spinor of the next tile: its buffer is released after this tile's hops
+          int next = tile, nr = rhs + 1;
+          if (nr == nrhs) { nr = 0; next = tile + gridDim.x; }
+          if (next < g.ntiles) {  // spinor of the next pass: its buffer is released after this pass's hops
             mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
-              bulk_g2s(sp + (p * 12) * TV, a.in + field_offset(g, 12, p, next, 0, 0), sp_bytes, &bars->full_sp);
+              bulk_g2s(sp + (p * 12) * TV, a.in + nr * a.rhs_stride + field_offset(g, 12, p, next, 0, 0), sp_bytes,
+                       &bars->full_sp);
           }
         }
       }
@@ -580,11 +588,13 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       // ------------------------------ halo loaders: LDGSTS one stage ahead ----------------------------
       const int lt = tid - (PIPE_CONS_WARPS + 1) * 32;
       RingPos hp = {0, 0u};   // halo buffer ring
-      for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x) {
+      for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+      for (int rhs = 0; rhs < nrhs; rhs++) {
         const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
+        const T2<T>* in_r = a.in + rhs * a.rhs_stride;
         for (int mu = 0; mu < 4; mu++) {
           mbar_wait_relaxed(&bars->empty_h[hp.slot], hp.ph ^ 1u);
-          halo_load<T, NCU>(g, a, tab, mu, halo + hp.slot * PIPE_NF, lt);
+          halo_load<T, NCU>(g, a, in_r, tab, mu, halo + hp.slot * PIPE_NF, lt);
           cp_async_arrive_noinc(&bars->full_h[hp.slot]);
           hp.advance(nhb);
         }
@@ -605,7 +615,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     RingPos rp = {0, 0u};
     RingPos hp = {0, 0u};
     int k = 0;
-    for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x, k++) {
+    for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+    for (int rhs = 0; rhs < nrhs; rhs++, k++) {
       const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
       const int x3 = __ldg(tab + 8) + l[3];
       const bool live = !(nonper && frozen_slice(g, x3));
@@ -682,7 +693,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         for (int c = 0; c < 12; c++) res[c] = cx<T>(0, 0);
       }
       // epilogue (same three variants as dw_kernel)
-      const size_t ooff = field_offset(g, 12, p, tile, 0, j);
+      const size_t ooff = field_offset(g, 12, p, tile, 0, j) + (size_t)(rhs * a.rhs_stride);
       if (a.epi == EPI_AXPY_NORM) {
         const T al = (T)(*a.alpha);
         T2<T>* rq = a.r + ooff;
@@ -919,6 +930,19 @@ cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cu
       if (recon == 12) return diag == DIAG_ONE ? launch_pipe<T, 12, DIAG_ONE>(g, a, c, s) : launch_pipe<T, 12, DIAG_PRE>(g, a, c, s);
       return diag == DIAG_ONE ? launch_pipe<T, 18, DIAG_ONE>(g, a, c, s) : launch_pipe<T, 18, DIAG_PRE>(g, a, c, s);
     }
+  }
+  if (a.nrhs > 1) {   // the one-thread-per-site kernels take one right-hand side per launch
+    for (int n = 0; n < a.nrhs; n++) {
+      DwArgs<T> b = a;
+      b.nrhs = 0;
+      b.in = a.in + n * a.rhs_stride;
+      b.self = (a.self == a.in) ? b.in : a.self + n * a.rhs_stride;
+      b.out = a.out + n * a.rhs_stride;
+      if (a.r) b.r = a.r + n * a.rhs_stride;
+      cudaError_t e = launch_dw<T>(g, b, recon, diag, s);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
   }
   if (recon == 12) {
     if (diag == DIAG_ONE) return launch_one<T, 12, DIAG_ONE>(g, a, s);

@@ -24,6 +24,8 @@ struct DwArgs {
   int dagger;
   int parity;                          // -1: both parities; 0/1: only this output parity
   int epi;
+  int nrhs;                            // > 1: in / out are arrays of nrhs spinor fields rhs_stride complex numbers apart
+  long long rhs_stride;                //      (several right-hand sides share the links and the clover term)
 };
 
 // number of per-CTA partial sums an EPI_*_NORM launch with these arguments writes to DwArgs::partial

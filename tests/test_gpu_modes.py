@@ -101,3 +101,39 @@ def test_plan_and_option_errors():
     small = Lattice((12, 6, 10, 8))    # extents not divisible by 4: no 4^4 tiles, the pipeline does not apply
     assert "dw_pipe_kernel" not in B.dw_plan(small.g)
     small.close()
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_dw_apply_multi(mode, prec):
+    """several right-hand sides in one pass share the links and clover blocks; the result
+    is the oracle's for every column and bit-identical to separate lqcd_dw_apply calls."""
+    L, bc, theta, kappa, csw, nrhs = (8, 4, 8, 12), B.BC_OPEN, (0.5, 0.5, 0.5, 0.0), 0.137, 1.9, 3
+    U = synth.smooth_gauge(L, 81)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
+    psis = [synth.gaussian_spinor(L, 82 + n) for n in range(nrhs)]
+    Uo, Ao = (round_f32(U), round_f32(A)) if prec == B.F32 else (U, A)
+    lat = Lattice(L, bc, theta)
+    lat.set_gauge(U, precs=(prec,))
+    lat.build_clover(kappa, csw, precs=(prec,))
+    fb = B.field_bytes(lat.g, B.FIELD_SPINOR, prec)
+    src = torch.empty(nrhs * fb, dtype=torch.uint8, device="cuda")
+    dst = torch.full((nrhs * fb,), 0x7F, dtype=torch.uint8, device="cuda")
+    for n in range(nrhs):
+        src[n * fb:(n + 1) * fb].copy_(lat.spinor(psis[n], prec))
+    mask = interior(L, bc)
+    for dagger in (False, True):
+        B.dw_apply_multi(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src, dst, nrhs, prec, dagger=dagger)
+        for n in range(nrhs):
+            got = lat.spinor_to_host(dst[n * fb:(n + 1) * fb], prec)
+            po = round_f32(psis[n]) if prec == B.F32 else psis[n]
+            ref = oracle.dw(L, Uo, po, kappa, Ao, bc=bc, theta=theta, dagger=dagger)
+            assert site_rel_err(got, ref, mask) <= TOL[prec]
+            single = lat.alloc(B.FIELD_SPINOR, prec)
+            fn = B.dwdag_apply if dagger else B.dw_apply
+            fn(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src[n * fb:(n + 1) * fb], single, prec)
+            torch.cuda.synchronize()
+            assert torch.equal(single, dst[n * fb:(n + 1) * fb])
+    with pytest.raises(B.LqcdError):   # overlapping arrays
+        B.dw_apply_multi(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src, src[fb:], 2, prec)
+    lat.close()
