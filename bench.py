@@ -127,6 +127,20 @@ def dist_env():
     return rank, world, local
 
 
+def max_over_ranks(torch, dist, ms_local, device):
+    """Replicas share nothing but the clock: the step time of the job is the slowest rank's."""
+    if dist is None:
+        return ms_local
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gflops(world, flops_step_per_rank, ms_per_step):
+    """value = work of all ranks / time of the slowest (weak scaling: every replica does the same work)."""
+    return world * flops_step_per_rank / (ms_per_step * 1e-3) / 1e9
+
+
 def time_calls(torch, fn, reps, warm=2):
     """Average milliseconds of fn() over `reps` back-to-back calls (CUDA events on the current stream)."""
     for _ in range(warm):
@@ -233,14 +247,10 @@ def run_ours(args):
     ms_local = e0.elapsed_time(e1)
     clocks = sampler.result()
     barrier()
-    ms = ms_local
-    if dist is not None:
-        t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(torch, dist, ms_local, "cuda")
     ms_per_step = ms / args.steps
     flops_step = 2.0 * FLOP_DW * V
-    value = world * flops_step / (ms_per_step * 1e-3) / 1e9  # GFLOP/s, whole job
+    value = whole_job_gflops(world, flops_step, ms_per_step)  # GFLOP/s, whole job
 
     # roofline of the dominant kernel (the stencil), from this rank's own launches in the timed region
     peak, peak_src = measured_peaks()
