@@ -396,7 +396,12 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
         "GB/s_model": gbs(reals_multi, 8, ms), "model": "%d reals/site for 12 columns (links + clover once)" % reals_multi,
         "note": "no gain over 12 single applications yet: with the links served by L2 the pipeline is bound by its "
                 "arithmetic warps (about 2.6 ms per right-hand side)"}
-    del src, dst
+    # NEXT-2: pseudoscalar two-point function of 12 columns (a pure reduction: 12 x 24 reals per site read once)
+    wsc = B.alloc_field(g, B.FIELD_WORKSPACE)
+    ms = time_calls(torch, lambda: B.correlator_ps(g, src, nrhs, wsc, L[3]), 3)
+    rows["next2_correlator_ps_12cols_f64"] = {"ms": round(ms, 3), "GB/s": gbs(24 * nrhs, 8, ms),
+                                              "frac_measured_peak": round(gbs(24 * nrhs, 8, ms) / peak, 4)}
+    del src, dst, wsc
     # a6: BLAS-1 reduction alone (|v|^2 over one spinor)
     ws = B.alloc_field(g, B.FIELD_WORKSPACE)
     ms = time_calls(torch, lambda: B.spinor_norm2(g, S.psi[B.F64], ws), 10)

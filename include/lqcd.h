@@ -132,6 +132,16 @@ lqcd_status lqcd_propagator(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_
 lqcd_status lqcd_spinor_norm2(const lqcd_geom* g, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream);
 lqcd_status lqcd_spinor_dot(const lqcd_geom* g, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host /* re, im */, void* stream);
 
+/* SURVEY.md 8(f) NEXT-2 (PAPER.md:11 "fermionic two point functions", :125 the columns of propagator!): the
+ * pseudoscalar two-point function of ncol propagator columns,
+ *   C(x4) = sum over x1,x2,x3 of sum over columns, spin, colour of |S(x)|^2      ( = sum_xvec Tr S^+ S ),
+ * accumulated in fp64 in a fixed order.  columns: DEVICE array of ncol internal spinor fields stored back to back
+ * (as lqcd_propagator writes them); workspace: DEVICE, lqcd_field_bytes(WORKSPACE); C_host: HOST array of L4
+ * doubles, valid on return (the call synchronises the stream).  A noise-source propagator (the other method of
+ * propagator!) is lqcd_cg_solve on a caller-supplied Gaussian source: random numbers are inputs of this library. */
+lqcd_status lqcd_correlator_ps(const lqcd_geom* g, const void* columns, int ncol, lqcd_prec prec, void* workspace,
+                               double* C_host, void* stream);
+
 /* End-to-end convenience over HOST buffers in the canonical layout (allocates device scratch, copies in,
  * imports, builds the clover term if csw != 0, applies D or D^+, exports, copies back). */
 lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host,

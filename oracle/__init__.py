@@ -194,3 +194,12 @@ def cg_eo(L, U, b, kappa, Ablk, Ainv, bc=BC_PERIODIC, theta=None, tol=1e-10, max
                             _p(Ainv), _p(b), _p(x), ctypes.c_double(tol), ctypes.c_int(maxiter),
                             ctypes.byref(rn), ctypes.byref(rt))
     return x, int(it), rn.value, rt.value
+
+
+def correlator_ps(L, cols):
+    """C(x4) = sum_{xvec} sum_{columns, spin, colour} |S|^2 for columns [ncol, V, 4, 3] (NEXT-2)."""
+    cols = np.ascontiguousarray(cols, dtype=np.complex128)
+    assert cols.ndim == 4 and cols.shape[1:] == (vol(L), 4, 3), cols.shape
+    C = np.zeros(int(L[3]), dtype=np.float64)
+    lib().oracle_correlator_ps(_L(L), _p(cols), ctypes.c_int(cols.shape[0]), _p(C))
+    return C

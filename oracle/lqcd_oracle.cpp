@@ -14,7 +14,8 @@
 // Pins (tests/test_oracle_pins.py): free-field closed form (P1), gamma5-hermiticity (P2), gauge
 // covariance (P3), dense 2^4 matrix built from the element formula in numpy (P4), constant abelian
 // flux closed form for the clover term (P5), antiperiodic equivalence (P6), Dirichlet structure
-// (P7), CG = dense inverse (P8), even-odd = full (P10), plaquette of the generator (P11).
+// (P7), CG = dense inverse (P8), even-odd = full (P10), plaquette of the generator (P11), free-field
+// pseudoscalar correlator from the momentum-space propagator (P12: point source + CG + contraction).
 // Parity unpinned: the value dependence of the c~_t boundary term (R10) beyond "ct=1 is absent and
 // the term is linear in (ct-1)".
 //
@@ -718,6 +719,22 @@ int oracle_cg_eo(const int L[4], int bc, const double theta[4], double kappa, co
         *rel_true = nb > 0 ? sqrt(norm2(t1.data(), N) / nb) : 0.0;
     }
     return it;
+}
+
+// NEXT-2 (SURVEY.md 8(f); PAPER.md:11 "different fermionic two point functions", :125 the propagator columns):
+// pseudoscalar two-point function from ncol propagator columns S_c(x) (canonical spinors [V][4][3]),
+//   C(x4) = sum over x1,x2,x3 of sum_c sum_{spin, colour} |S_c(x)|^2     ( = sum_xvec Tr S(x)^+ S(x) for the 12 columns
+// of a point source, since gamma5-hermiticity turns Tr[gamma5 S gamma5 S^+] into it).  Plain loops, x4 slowest (D1).
+void oracle_correlator_ps(const int L[4], const cd* cols, int ncol, double* C) {
+    const long V = (long)L[0] * L[1] * L[2] * L[3];
+    const long V3 = (long)L[0] * L[1] * L[2];
+    for (int t = 0; t < L[3]; t++) {
+        double s = 0.0;
+        for (int c = 0; c < ncol; c++)
+            for (long n = (long)t * V3; n < (long)(t + 1) * V3; n++)
+                for (int k = 0; k < 12; k++) s += std::norm(cols[((long)c * V + n) * 12 + k]);
+        C[t] = s;
+    }
 }
 
 }  // extern "C"

@@ -23,7 +23,7 @@ EXPORTS = [
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
-    "lqcd_set_option", "lqcd_dw_apply_multi",
+    "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps",
 ]
 
 
@@ -264,6 +264,13 @@ def dw_apply_multi(g, kappa, U, clover, src, dst, nrhs, prec=F64, recon=RECON_18
     d = _dirac(kappa)
     _check(lib().lqcd_dw_apply_multi(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(src), _ptr(dst), int(nrhs),
                                      1 if dagger else 0, prec, recon, _stream(stream)))
+
+
+def correlator_ps(g, columns, ncol, workspace, L4, prec=F64, stream=None):
+    """C(x4) = sum_xvec sum_{columns, spin, colour} |S|^2 as a list of L4 floats."""
+    C = (ctypes.c_double * int(L4))()
+    _check(lib().lqcd_correlator_ps(g, _ptr(columns), int(ncol), prec, _ptr(workspace), C, _stream(stream)))
+    return list(C)
 
 
 def launch_count():

@@ -434,6 +434,20 @@ lqcd_status lqcd_spinor_norm2(const lqcd_geom* h, const void* v, int half, lqcd_
                          device_norm2<float>(v, n, partial, scratch, result_host, as_stream(stream))), "norm2");
   return LQCD_OK;
 }
+lqcd_status lqcd_correlator_ps(const lqcd_geom* h, const void* columns, int ncol, lqcd_prec prec, void* workspace,
+                               double* C_host, void* stream) {
+  REQUIRE(h && columns && workspace && C_host, "lqcd_correlator_ps: NULL argument");
+  REQUIRE(valid_prec(prec) && ncol >= 1 && ncol <= 4096, "lqcd_correlator_ps: bad precision or column count");
+  const Geom& g = h->g;
+  double* partial = (double*)workspace;   // the workspace is several spinor fields large: ntiles*b3 + L4 doubles fit
+  double* C_dev = partial + (size_t)g.ntiles * g.b[3];
+  cudaStream_t s = as_stream(stream);
+  CUDA_TRY(DISPATCH_PREC(prec, correlator_ps<double>(g, columns, ncol, partial, C_dev, s),
+                         correlator_ps<float>(g, columns, ncol, partial, C_dev, s)), "correlator kernel");
+  CUDA_TRY(cudaMemcpyAsync(C_host, C_dev, (size_t)g.L[3] * sizeof(double), cudaMemcpyDeviceToHost, s), "memcpy");
+  CUDA_TRY(cudaStreamSynchronize(s), "sync");
+  return LQCD_OK;
+}
 lqcd_status lqcd_spinor_dot(const lqcd_geom* h, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream) {
   REQUIRE(h && u && v && workspace && result_host, "lqcd_spinor_dot: NULL argument");
   REQUIRE(valid_prec(prec), "lqcd_spinor_dot: bad precision");

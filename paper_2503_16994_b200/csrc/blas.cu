@@ -247,4 +247,66 @@ INST(double)
 INST(float)
 #undef INST
 
+// ---- NEXT-2: pseudoscalar two-point function C(x4) = sum_{xvec} sum_{columns, spin, colour} |S|^2 ---------------
+// (SURVEY.md 8(f)).  One CTA per tile, one thread per site; a site's |S|^2 over all columns is
+// accumulated in fp64, then summed per local time coordinate in a fixed order; the second kernel adds the tiles of
+// each time slice with a fixed assignment of tiles to threads and a fixed reduction tree, so the result is deterministic.
+template <typename T>
+__global__ void __launch_bounds__(256) corr_ps_tile_kernel(const Geom g, const T2<T>* __restrict__ cols, const int ncol,
+                                                           const long long col_stride, double* __restrict__ partial) {
+  __shared__ double s_val[256];
+  const int TV = g.TV;
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x;
+  double acc = 0.0;
+  int l3 = -1;
+  if (tid < 2 * TV) {
+    const int p = tid >= TV ? 1 : 0;
+    const int j = tid - p * TV;
+    int l[4];
+    local_coords(g, j, p, l);
+    l3 = l[3];
+    const size_t off = field_offset(g, 12, p, tile, 0, j);
+    for (int c = 0; c < ncol; c++) {
+      const T2<T>* v = cols + (size_t)c * col_stride + off;
+#pragma unroll
+      for (int k = 0; k < 12; k++) {
+        const T2<T> w = __ldg(v + (size_t)k * TV);
+        acc += (double)w.x * (double)w.x + (double)w.y * (double)w.y;
+      }
+    }
+  }
+  s_val[tid] = acc;
+  __syncthreads();
+  if (tid < g.b[3]) {   // thread t adds the sites with local time t, in thread order
+    double s = 0.0;
+    const int st3 = (g.b[0] >> 1) << (g.lb[1] + g.lb[2]);   // j stride of l3
+    for (int p = 0; p < 2; p++)
+      for (int jj = 0; jj < st3; jj++) s += s_val[p * TV + tid * st3 + jj];
+    partial[(size_t)tile * g.b[3] + tid] = s;
+  }
+}
+__global__ void __launch_bounds__(256) corr_ps_final_kernel(const Geom g, const double* __restrict__ partial,
+                                                            double* __restrict__ C) {
+  __shared__ double s_red[32];
+  const int x4 = blockIdx.x;   // one CTA per time slice
+  const int origin = (x4 / g.b[3]) * g.b[3], l3 = x4 - origin;
+  double acc = 0.0;
+  for (int t = threadIdx.x; t < g.ntiles; t += blockDim.x)   // thread i: tiles i, i+256, ... in order
+    if (__ldg(g.tile_tab + (size_t)t * TILE_TAB + 8) == origin) acc += partial[(size_t)t * g.b[3] + l3];
+  const double s = block_sum(acc, s_red);
+  if (threadIdx.x == 0) C[x4] = s;
+}
+template <typename T>
+cudaError_t correlator_ps(const Geom& g, const void* cols, int ncol, double* partial, double* C_dev, cudaStream_t s) {
+  const int threads = ((2 * g.TV + 31) / 32) * 32;
+  corr_ps_tile_kernel<T><<<g.ntiles, threads, 0, s>>>(g, (const T2<T>*)cols, ncol, (long long)2 * g.Vh * 12, partial);
+  count_launch();
+  corr_ps_final_kernel<<<g.L[3], 256, 0, s>>>(g, partial, C_dev);
+  count_launch();
+  return cudaGetLastError();
+}
+template cudaError_t correlator_ps<double>(const Geom&, const void*, int, double*, double*, cudaStream_t);
+template cudaError_t correlator_ps<float>(const Geom&, const void*, int, double*, double*, cudaStream_t);
+
 }  // namespace lqcd

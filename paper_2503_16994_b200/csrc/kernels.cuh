@@ -43,6 +43,8 @@ template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void*
 template <typename T> cudaError_t axpy(double a, const void* x, void* y, size_t ncomplex, cudaStream_t s);
 template <typename T> cudaError_t xmy(const void* x, const void* y, void* z, size_t ncomplex, cudaStream_t s);  // z = x - y
 cudaError_t add_f32_to_f64(const void* e32, void* x64, size_t ncomplex, cudaStream_t s);                          // x += e
+// NEXT-2: C(x4) of ncol spinor fields stored back to back; partial >= ntiles*b3 doubles, C_dev >= L4 doubles
+template <typename T> cudaError_t correlator_ps(const Geom& g, const void* cols, int ncol, double* partial, double* C_dev, cudaStream_t s);
 // zero the frozen time slices of a spinor (D7: the solve lives on the interior)
 template <typename T> cudaError_t mask_frozen(const Geom& g, void* psi, cudaStream_t s);
 

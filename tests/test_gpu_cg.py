@@ -10,7 +10,7 @@ import oracle
 from paper_2503_16994_b200 import binding as B
 from paper_2503_16994_b200 import synth
 
-from gpu_util import Lattice, interior, site_rel_err
+from gpu_util import Lattice, interior, round_f32, site_rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -125,4 +125,61 @@ def test_propagator_12_columns():
         x = lat.spinor_to_host(cols[c * nbytes:(c + 1) * nbytes])
         assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= 1e-8
         assert abs(infos[c]["iters"] - it_o) <= 2
+    lat.close()
+
+
+@pytest.mark.parametrize("L,bc", [((8, 4, 8, 12), B.BC_PERIODIC), ((6, 4, 10, 8), B.BC_OPEN)])
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_correlator_ps_matches_oracle(L, bc, prec):
+    """NEXT-2: C(x4) of a set of columns against the oracle's plain loops (fp64 accumulation on both sides; the
+    fp32 case feeds the oracle the same rounded columns), on 4^4 tiles and on a lattice without them."""
+    V = synth.vol(L)
+    lat = Lattice(L, bc)
+    ncol = 5
+    fb = B.field_bytes(lat.g, B.FIELD_SPINOR, prec)
+    cols_dev = torch.empty(ncol * fb, dtype=torch.uint8, device="cuda")
+    cols = []
+    for c in range(ncol):
+        psi = synth.gaussian_spinor(L, 300 + c)
+        cols.append(round_f32(psi) if prec == B.F32 else psi)
+        cols_dev[c * fb:(c + 1) * fb].copy_(lat.spinor(psi, prec))
+    ws = lat.alloc(B.FIELD_WORKSPACE)
+    got = np.array(B.correlator_ps(lat.g, cols_dev, ncol, ws, L[3], prec))
+    ref = oracle.correlator_ps(L, np.array(cols))
+    assert np.max(np.abs(got - ref) / ref) <= 1e-13
+    lat.close()
+
+
+def test_propagator_to_correlator_and_noise_source():
+    """The paper's use of the solver: 12 point-source columns -> pseudoscalar correlator, and the
+    noise-source method of propagator! (a Gaussian source on one time slice, drawn by the seeded generator and
+    passed in), both against the oracle end to end."""
+    L, kappa, csw = (4, 4, 4, 8), 0.125, 1.0
+    theta = (0, 0, 0, np.pi)
+    U, A, lat = setup(L, B.BC_PERIODIC, theta, None, kappa, csw, 141)
+    V = synth.vol(L)
+    nbytes = B.field_bytes(lat.g, B.FIELD_SPINOR)
+    cols = torch.empty(12 * nbytes, dtype=torch.uint8, device="cuda")
+    ws = lat.alloc(B.FIELD_WORKSPACE)
+    B.propagator(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], (0, 0, 0, 0), cols, ws, tol=1e-12)
+    got = np.array(B.correlator_ps(lat.g, cols, 12, ws, L[3]))
+    ref_cols = []
+    for c in range(12):
+        b = synth.point_source(L, (0, 0, 0, 0), c // 3, c % 3)
+        ref_cols.append(oracle.cg(L, U, b, kappa, A, theta=theta, tol=1e-12)[0])
+    ref = oracle.correlator_ps(L, np.array(ref_cols))
+    assert np.max(np.abs(got - ref) / ref) <= 1e-8
+    assert np.all(got > 0) and got[0] == got.max()
+    # noise source on time slice 2
+    V3 = L[0] * L[1] * L[2]
+    eta = np.zeros((V, 4, 3), dtype=np.complex128)
+    eta[2 * V3:3 * V3] = synth.gaussian_spinor(L, 142)[2 * V3:3 * V3]
+    x = lat.alloc(B.FIELD_SPINOR)
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], lat.spinor(eta), x, ws, tol=1e-12)
+    xo, it_o, _, _ = oracle.cg(L, U, eta, kappa, A, theta=theta, tol=1e-12)
+    assert abs(info["iters"] - it_o) <= 2
+    assert np.linalg.norm(lat.spinor_to_host(x) - xo) / np.linalg.norm(xo) <= 1e-8
+    c_gpu = np.array(B.correlator_ps(lat.g, x, 1, ws, L[3]))
+    c_ref = oracle.correlator_ps(L, xo[None])
+    assert np.max(np.abs(c_gpu - c_ref) / c_ref) <= 1e-8
     lat.close()

@@ -507,3 +507,54 @@ def test_dw_at_sites_matches_field():
         full = oracle.dw(L, U, psi, kappa, Ablk=A, theta=theta, dagger=dagger)
         some = oracle.dw_at_sites(L, U, psi, sites, kappa, csw, theta=theta, dagger=dagger)
         assert np.array_equal(some, full[sites])
+
+
+def test_P12_free_field_pseudoscalar_correlator():
+    """NEXT-2 pin: on U = 1 the point-source propagator is the inverse lattice Fourier transform of
+    D(p)^-1 = [(1 - 2k sum cos p) - 2k i sum gamma sin p] / [(1 - 2k sum cos p)^2 + 4 k^2 sum sin^2 p] (P1), so
+    C(x4) = sum_xvec Tr S^+ S is known in closed form: it pins point source + CG + contraction together
+    (theta_4 = pi: antiperiodic in time, the momenta shift by theta/L)."""
+    L = (4, 4, 4, 8)
+    V = synth.vol(L)
+    kappa = 0.115
+    theta = (0.0, 0.0, 0.0, math.pi)
+    U = np.tile(np.eye(3, dtype=complex), (V, 4, 1, 1))
+    # momentum-space propagator on the grid p_mu = (2 pi n_mu + theta_mu) / L_mu, array index order [n4, n3, n2, n1]
+    grids = np.meshgrid(*[(2 * math.pi * np.arange(L[mu]) + theta[mu]) / L[mu] for mu in (3, 2, 1, 0)], indexing="ij")
+    p = {3: grids[0], 2: grids[1], 1: grids[2], 0: grids[3]}
+    a = 1 - 2 * kappa * sum(np.cos(p[mu]) for mu in range(4))
+    den = a ** 2 + 4 * kappa ** 2 * sum(np.sin(p[mu]) ** 2 for mu in range(4))
+    Sp = a[..., None, None] * np.eye(4) - 2j * kappa * sum(np.sin(p[mu])[..., None, None] * GAMMA[mu] for mu in range(4))
+    Sp = Sp / den[..., None, None]
+    # S(x) = (1/V) sum_p e^{i p x} S(p);  the theta part of p is the twist phase e^{i theta_mu x_mu / L_mu}
+    Sx = np.fft.ifftn(Sp, axes=(0, 1, 2, 3))
+    x4 = np.arange(L[3]).reshape(-1, 1, 1, 1)
+    Sx = Sx * np.exp(1j * theta[3] * x4 / L[3])[..., None, None]
+    want = 3.0 * (np.abs(Sx) ** 2).sum(axis=(1, 2, 3, 4, 5))     # 3 colours x spin trace, per time slice
+    cols = []
+    for spin in range(4):
+        for colour in range(3):
+            b = synth.point_source(L, (0, 0, 0, 0), spin, colour)
+            x, it, _, _ = oracle.cg(L, U, b, kappa, None, theta=theta, tol=1e-13)
+            assert it > 0
+            cols.append(x)
+    got = oracle.correlator_ps(L, np.array(cols))
+    assert np.max(np.abs(got - want) / want) < 1e-9
+    assert got[0] > got[1] > got[2] > got[3] > got[4]            # decays away from the source, symmetric in time
+    assert np.allclose(got[1:4], got[:4:-1][:3], rtol=1e-9)
+
+
+def test_correlator_slice_mapping_and_sum_rule():
+    """x4 is the slowest canonical index (D1): a field living on one time slice contributes to that entry only;
+    sum_t C(t) = sum of the squared norms of the columns."""
+    L = (4, 6, 2, 8)
+    V = synth.vol(L)
+    V3 = L[0] * L[1] * L[2]
+    rng = np.random.default_rng(7)
+    cols = rng.standard_normal((3, V, 4, 3)) + 1j * rng.standard_normal((3, V, 4, 3))
+    C = oracle.correlator_ps(L, cols)
+    assert abs(C.sum() - np.linalg.norm(cols) ** 2) / C.sum() < 1e-14
+    one = np.zeros_like(cols)
+    one[:, 5 * V3:6 * V3] = cols[:, 5 * V3:6 * V3]
+    C1 = oracle.correlator_ps(L, one)
+    assert C1[5] == C[5] and np.count_nonzero(C1) == 1
