@@ -420,9 +420,32 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
                                    "model": "%d reals/site/iteration (fused plan, SURVEY.md 8(d))" % REALS_CG_ITER[recon]}
     del ws
     torch.cuda.empty_cache()
+    rows.update(run_config2(torch, B, synth, peak))
     rows.update(run_config3(torch, B, synth, peak))
     rows.update(run_config4(torch, B, synth, peak))
     return rows
+
+
+def run_config2(torch, B, synth, peak):
+    """configs[1]: 16^3 x 32 periodic, kappa = 0.135, csw = 1.7: 10 warm-up + 1000 applications of Dw to a fixed input,
+    fp64 and fp32.  The working set (192 / 96 MB) is about the size of L2, so this is not an HBM-roofline point."""
+    L, kappa, csw = (16, 16, 16, 32), 0.135, 1.7
+    S = Setup(torch, B, synth, L, B.BC_PERIODIC, None, None, kappa, csw, 2, 0, [B.F64, B.F32], [18])
+    g, V = S.g, S.V
+    U32 = B.alloc_field(g, B.FIELD_GAUGE, B.F32, 18)
+    B.field_to_f32(g, B.FIELD_GAUGE, 18, S.U[(B.F64, 18)], U32)
+    S.U[(B.F32, 18)] = U32
+    out = {}
+    for p, pname, rb in ((B.F64, "f64", 8), (B.F32, "f32", 4)):
+        ms = time_calls(torch, lambda: B.dw_apply(g, kappa, S.U[(p, 18)], S.A[p], S.psi[p], S.out[p], p, 18), 1000, 10)
+        gb = REALS_DW[18] * rb * V / (ms * 1e-3) / 1e9
+        out["a4_dw_16x16x16x32_%s_1000_applications" % pname] = {
+            "ms": round(ms, 5), "GFLOP/s": round(FLOP_DW * V / ms / 1e6, 1), "GB/s_model": round(gb, 1),
+            "note": "working set ~ L2 (%d MB): not an HBM roofline point" % (REALS_DW[18] * rb * V >> 20)}
+    S.close()
+    del S, U32
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_config3(torch, B, synth, peak):

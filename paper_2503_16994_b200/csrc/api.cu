@@ -215,13 +215,6 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   }
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device), "cudaGetDeviceProperties");
-  if (getenv("LQCD_L2_FETCH")) {   // experiment: DRAM -> L2 fetch granularity hint (32/64/128 bytes)
-    size_t before = 0, after = 0;
-    cudaDeviceGetLimit(&before, cudaLimitMaxL2FetchGranularity);
-    cudaError_t e = cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)atoi(getenv("LQCD_L2_FETCH")));
-    cudaDeviceGetLimit(&after, cudaLimitMaxL2FetchGranularity);
-    fprintf(stderr, "[lqcd] L2 fetch granularity %zu -> %zu (%s)\n", before, after, cudaGetErrorString(e));
-  }
   h->sm_count = prop.multiProcessorCount;
   h->smem_optin = (int)prop.sharedMemPerBlockOptin;
   g.sm_count = h->sm_count;

@@ -814,7 +814,7 @@ static DirectCfg direct_config_t(const Geom& g, int parity) {
   const int npar = parity < 0 ? 2 : 1;
   c.kind = KIND_FULL;
   if (parity < 0 && mode == MODE_SPLIT) c.kind = KIND_SPLIT;
-  else if (npar * g.TV <= 128 && env_int("LQCD_HALF3", 1)) c.kind = KIND_HALF;
+  else if (npar * g.TV <= 128) c.kind = KIND_HALF;
   c.threads = c.kind == KIND_SPLIT ? ((g.TV + 31) / 32) * 32 : ((npar * g.TV + 31) / 32) * 32;
   const int items = c.kind == KIND_SPLIT ? 2 * g.ntiles : g.ntiles;
   c.grid = items;
