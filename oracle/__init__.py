@@ -63,6 +63,19 @@ def _d(v, n):
     return (ctypes.c_double * n)(*[float(t) for t in v])
 
 
+class _twisted:
+    """Sets the oracle's twisted mass for the duration of one call (NEXT-4; 0 = plain Wilson-clover)."""
+
+    def __init__(self, mu):
+        self.mu = float(mu)
+
+    def __enter__(self):
+        lib().oracle_set_twisted_mass(ctypes.c_double(self.mu))
+
+    def __exit__(self, *exc):
+        lib().oracle_set_twisted_mass(ctypes.c_double(0.0))
+
+
 def vol(L):
     return int(L[0]) * int(L[1]) * int(L[2]) * int(L[3])
 
@@ -124,7 +137,8 @@ def clover_inverse(L, Ablk):
     return out
 
 
-def dw(L, U, psi, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, dagger=False):
+def dw(L, U, psi, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, dagger=False, mu=0.0):
+    """D psi (or D^+ psi); mu = twisted mass: D = A + 2 i kappa mu gamma5 - kappa H."""
     U = _c(U, (vol(L), 4, 3, 3))
     psi = _c(psi, (vol(L), 4, 3))
     out = np.zeros_like(psi)
@@ -132,8 +146,9 @@ def dw(L, U, psi, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, dagger=False):
     if Ablk is not None:
         Ablk = _c(Ablk, (vol(L), 2, 6, 6))
         ap = _p(Ablk)
-    lib().oracle_dw(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(psi),
-                    _p(out), ctypes.c_int(1 if dagger else 0))
+    with _twisted(mu):
+        lib().oracle_dw(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(psi),
+                        _p(out), ctypes.c_int(1 if dagger else 0))
     return out
 
 
@@ -167,7 +182,7 @@ def dhat(L, U, psi, kappa, Ablk, Ainv, bc=BC_PERIODIC, theta=None, dagger=False)
     return out
 
 
-def cg(L, U, b, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter=10000):
+def cg(L, U, b, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter=10000, mu=0.0):
     """Returns (x, iters, rel_resid_normal, rel_resid_true); iters < 0 means maxiter was hit."""
     U = _c(U, (vol(L), 4, 3, 3))
     b = _c(b, (vol(L), 4, 3))
@@ -177,9 +192,10 @@ def cg(L, U, b, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter
         Ablk = _c(Ablk, (vol(L), 2, 6, 6))
         ap = _p(Ablk)
     rn, rt = ctypes.c_double(0), ctypes.c_double(0)
-    it = lib().oracle_cg(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(b),
-                         _p(x), ctypes.c_double(tol), ctypes.c_int(maxiter), ctypes.byref(rn),
-                         ctypes.byref(rt))
+    with _twisted(mu):
+        it = lib().oracle_cg(_L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(b),
+                             _p(x), ctypes.c_double(tol), ctypes.c_int(maxiter), ctypes.byref(rn),
+                             ctypes.byref(rt))
     return x, int(it), rn.value, rt.value
 
 

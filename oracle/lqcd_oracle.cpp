@@ -43,7 +43,11 @@ struct Lat {
     long V;
     cd theta[4];      // per-link phase factor exp(i*angle/L_mu)   (D3, R6)
     double phiT[3];   // SF boundary phases at x4 = T               (D7, R8)
+    double mu;        // twisted mass ("mu is the twisted mass"): D = A + 2 i kappa mu gamma5 - kappa H
 };
+// NEXT-4: the twisted mass is a state of this library (oracle_set_twisted_mass), read when a lattice is set up;
+// the Python wrapper sets it before and clears it after each call.  Even-odd routines do not support it.
+static double g_twisted_mu = 0.0;
 
 // ----------------------------------------------------------------------------------------------
 // D2: gamma matrices, chiral basis.  gamma_k = [[0,-i sigma_k],[+i sigma_k,0]], gamma_4 = [[0,1],[1,0]]
@@ -131,6 +135,7 @@ static Lat make_lat(const int L[4], int bc, const double theta[4], const double 
         g.theta[i] = cd(cos(ang), sin(ang));
     }
     for (int i = 0; i < 3; i++) g.phiT[i] = phiT ? phiT[i] : 0.0;
+    g.mu = g_twisted_mu;
     init_gamma();
     return g;
 }
@@ -351,6 +356,16 @@ static void dw_site(const Lat& g, const cd* U, const cd* Ablk, const cd* psi, co
             }
     }
     for (int i = 0; i < 12; i++) r[i] -= kappa * h[i];
+    if (g.mu != 0.0) {
+        // + 2 i kappa mu gamma5 psi; D^dagger = gamma5 D(-mu) gamma5, so the conjugated path (g5) carries -mu
+        const double m = 2.0 * kappa * (g5 ? -g.mu : g.mu);
+        for (int s = 0; s < 4; s++)
+            for (int a = 0; a < 3; a++) {
+                cd v = 0;
+                for (int sp = 0; sp < 4; sp++) v += GAM5[s][sp] * p[3 * sp + a];
+                r[3 * s + a] += I_ * m * v;
+            }
+    }
     if (g5) {
         for (int s = 0; s < 4; s++)
             for (int a = 0; a < 3; a++) {
@@ -534,6 +549,8 @@ static int cg_normal(long N, Op M, const cd* b, cd* x, double tol, int maxiter, 
 // C-ABI
 // ----------------------------------------------------------------------------------------------
 extern "C" {
+
+void oracle_set_twisted_mass(double mu) { g_twisted_mu = mu; }
 
 int oracle_num_threads(void) {
 #ifdef _OPENMP

@@ -558,3 +558,51 @@ def test_correlator_slice_mapping_and_sum_rule():
     one[:, 5 * V3:6 * V3] = cols[:, 5 * V3:6 * V3]
     C1 = oracle.correlator_ps(L, one)
     assert C1[5] == C[5] and np.count_nonzero(C1) == 1
+
+
+@pytest.mark.parametrize("mu", [0.05, -0.3])
+def test_P13_twisted_mass(mu):
+    """NEXT-4 pin ("mu is the twisted mass"): D = A + 2 i kappa mu gamma5 - kappa H.
+    Free field: D(p) = a + 2 i kappa (gamma.sin p) + 2 i kappa mu gamma5 and D^+ D = a^2 + 4 k^2 sum sin^2 + (2 k mu)^2
+    (gamma5 anticommutes with every gamma_mu, so the cross terms cancel); D(mu)^+ = gamma5 D(-mu) gamma5 on an
+    interacting field; and the term is exactly the difference to mu = 0."""
+    L = (4, 4, 6, 4)
+    V = synth.vol(L)
+    kappa = 0.124
+    U1 = np.tile(np.eye(3, dtype=complex), (V, 4, 1, 1))
+    n = np.arange(V)
+    xs = [n % L[0], (n // L[0]) % L[1], (n // (L[0] * L[1])) % L[2], n // (L[0] * L[1] * L[2])]
+    rng = np.random.default_rng(5)
+    for mom in [(0, 0, 0, 0), (1, 3, 2, 1), (2, 0, 5, 3)]:
+        p = [2 * math.pi * mom[m] / L[m] for m in range(4)]
+        u = rng.standard_normal(12) + 1j * rng.standard_normal(12)
+        phase = np.exp(1j * sum(p[m] * xs[m] for m in range(4)))
+        psi = (phase[:, None] * u[None, :]).reshape(V, 4, 3)
+        a = 1 - 2 * kappa * sum(math.cos(t) for t in p)
+        gs = sum(math.sin(p[m]) * GAMMA[m] for m in range(4))
+        Dm = np.kron(a * np.eye(4) + 2j * kappa * gs + 2j * kappa * mu * GAMMA5, np.eye(3))
+        want = (phase[:, None] * (Dm @ u)[None, :]).reshape(V, 4, 3)
+        got = oracle.dw(L, U1, psi, kappa, mu=mu)
+        assert np.linalg.norm(got - want) / np.linalg.norm(psi) < 1e-14
+        wantd = (phase[:, None] * (Dm.conj().T @ u)[None, :]).reshape(V, 4, 3)
+        assert np.linalg.norm(oracle.dw(L, U1, psi, kappa, mu=mu, dagger=True) - wantd) / np.linalg.norm(psi) < 1e-14
+        dd = a ** 2 + 4 * kappa ** 2 * sum(math.sin(t) ** 2 for t in p) + (2 * kappa * mu) ** 2
+        assert np.linalg.norm(oracle.dw(L, U1, got, kappa, mu=mu, dagger=True) - dd * psi) / np.linalg.norm(psi) < 1e-14
+    # interacting field with clover term
+    U = synth.smooth_gauge(L, 97)
+    A = oracle.clover_blocks(L, U, kappa, 1.6)
+    psi = synth.gaussian_spinor(L, 98)
+    chi = synth.gaussian_spinor(L, 99)
+    g5 = lambda v: v * np.array([1, 1, -1, -1])[None, :, None]
+    lhs = oracle.dw(L, U, psi, kappa, A, mu=mu, dagger=True)
+    rhs = g5(oracle.dw(L, U, g5(psi), kappa, A, mu=-mu))
+    assert np.linalg.norm(lhs - rhs) / np.linalg.norm(rhs) < 1e-14
+    # <chi, D psi> = <D^+ chi, psi>
+    a1 = np.vdot(chi, oracle.dw(L, U, psi, kappa, A, mu=mu))
+    a2 = np.vdot(oracle.dw(L, U, chi, kappa, A, mu=mu, dagger=True), psi)
+    assert abs(a1 - a2) / abs(a1) < 1e-13
+    diff = oracle.dw(L, U, psi, kappa, A, mu=mu) - oracle.dw(L, U, psi, kappa, A)
+    assert np.linalg.norm(diff - 2j * kappa * mu * g5(psi)) / np.linalg.norm(psi) < 1e-15
+    # CG on the normal equations of the twisted operator
+    x, it, rn, rt = oracle.cg(L, U, psi, kappa, A, tol=1e-11, mu=mu)
+    assert it > 0 and np.linalg.norm(oracle.dw(L, U, x, kappa, A, mu=mu) - psi) / np.linalg.norm(psi) < 1e-9
