@@ -63,8 +63,11 @@ typedef struct {
   int device;          /* CUDA ordinal                                                                   */
 } lqcd_geom_desc;
 
-/* Dirac parameters: kappa = 1/(2(m0+4)); csw; ct = c~_t (paper's cF), 1 = absent. */
-typedef struct { double kappa, csw, ct; } lqcd_dirac;
+/* Dirac parameters: kappa = 1/(2(m0+4)); csw; ct = c~_t (paper's cF), 1 = absent; mu = twisted
+ * mass: D = A + 2 i kappa mu gamma5 - kappa H, D^+ = gamma5 D(-mu) gamma5; 0 = absent.
+ * mu != 0 is supported by lqcd_dw_apply / lqcd_dwdag_apply / lqcd_dw_apply_multi / lqcd_dw_apply_host and by the
+ * plain (not even-odd) lqcd_cg_solve / lqcd_propagator; the even-odd paths return LQCD_EINVAL for mu != 0. */
+typedef struct { double kappa, csw, ct, mu; } lqcd_dirac;
 
 typedef struct lqcd_geom lqcd_geom;   /* opaque, library-owned */
 

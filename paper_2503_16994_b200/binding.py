@@ -39,7 +39,8 @@ class GeomDesc(ctypes.Structure):
 
 
 class Dirac(ctypes.Structure):
-    _fields_ = [("kappa", ctypes.c_double), ("csw", ctypes.c_double), ("ct", ctypes.c_double)]
+    _fields_ = [("kappa", ctypes.c_double), ("csw", ctypes.c_double), ("ct", ctypes.c_double),
+                ("mu", ctypes.c_double)]
 
 
 class CgParm(ctypes.Structure):
@@ -102,8 +103,8 @@ def _stream(stream):
     return ctypes.c_void_p(stream.cuda_stream)
 
 
-def _dirac(kappa, csw=0.0, ct=1.0):
-    return Dirac(float(kappa), float(csw), float(ct))
+def _dirac(kappa, csw=0.0, ct=1.0, mu=0.0):
+    return Dirac(float(kappa), float(csw), float(ct), float(mu))
 
 
 def geom_desc(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0):
@@ -176,14 +177,14 @@ def clover_build(g, kappa, csw, U64, clover, clover_inv=None, recon=RECON_18, ou
                                    _stream(stream)))
 
 
-def dw_apply(g, kappa, U, clover, psi_in, psi_out, prec=F64, recon=RECON_18, stream=None):
-    d = _dirac(kappa)
+def dw_apply(g, kappa, U, clover, psi_in, psi_out, prec=F64, recon=RECON_18, stream=None, mu=0.0):
+    d = _dirac(kappa, mu=mu)
     _check(lib().lqcd_dw_apply(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(psi_in), _ptr(psi_out), prec, recon,
                                _stream(stream)))
 
 
-def dwdag_apply(g, kappa, U, clover, psi_in, psi_out, prec=F64, recon=RECON_18, stream=None):
-    d = _dirac(kappa)
+def dwdag_apply(g, kappa, U, clover, psi_in, psi_out, prec=F64, recon=RECON_18, stream=None, mu=0.0):
+    d = _dirac(kappa, mu=mu)
     _check(lib().lqcd_dwdag_apply(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(psi_in), _ptr(psi_out), prec, recon,
                                   _stream(stream)))
 
@@ -212,9 +213,9 @@ def _info_dict(info, status):
 
 def cg_solve(g, kappa, U64, clover64, b, x, workspace, tol=1e-10, maxiter=10000, clover_inv64=None, U32=None,
              clover32=None, clover_inv32=None, mixed=False, eo=False, inner_tol=1e-4, check_every=16,
-             recon=RECON_18, stream=None, raise_on_notconv=True):
+             recon=RECON_18, stream=None, raise_on_notconv=True, mu=0.0):
     """Returns a dict (iters, outer, rel_resid_normal, rel_resid_true, seconds, status)."""
-    d = _dirac(kappa)
+    d = _dirac(kappa, mu=mu)
     f, p = _cg_args(U64, clover64, clover_inv64, U32, clover32, clover_inv32, tol, maxiter, mixed, eo, inner_tol, check_every)
     info = CgInfo()
     st = lib().lqcd_cg_solve(g, ctypes.byref(d), ctypes.byref(f), _ptr(b), _ptr(x), _ptr(workspace), ctypes.byref(p),
@@ -226,9 +227,9 @@ def cg_solve(g, kappa, U64, clover64, b, x, workspace, tol=1e-10, maxiter=10000,
 
 def propagator(g, kappa, U64, clover64, y, columns, workspace, tol=1e-10, maxiter=10000, clover_inv64=None, U32=None,
                clover32=None, clover_inv32=None, mixed=False, eo=False, inner_tol=1e-4, check_every=16,
-               recon=RECON_18, stream=None):
+               recon=RECON_18, stream=None, mu=0.0):
     """12 point-source columns (spin-major: column = 3*spin + colour) into `columns` (12 internal fp64 spinors)."""
-    d = _dirac(kappa)
+    d = _dirac(kappa, mu=mu)
     f, p = _cg_args(U64, clover64, clover_inv64, U32, clover32, clover_inv32, tol, maxiter, mixed, eo, inner_tol, check_every)
     infos = (CgInfo * 12)()
     yy = (ctypes.c_int * 4)(*[int(v) for v in y])
@@ -251,17 +252,17 @@ def spinor_dot(g, u, v, workspace, half=False, prec=F64, stream=None):
 
 
 def dw_apply_host(L, kappa, csw, U_canon, psi_canon, out_canon, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None,
-                  dagger=False, prec=F64, recon=RECON_18, ct=1.0, device=0):
+                  dagger=False, prec=F64, recon=RECON_18, ct=1.0, device=0, mu=0.0):
     """End to end over HOST buffers (numpy complex128, canonical layout); copies are inside the call."""
     desc = geom_desc(L, bc, theta, phi0, phiT, device)
-    d = _dirac(kappa, csw, ct)
+    d = _dirac(kappa, csw, ct, mu)
     _check(lib().lqcd_dw_apply_host(ctypes.byref(desc), ctypes.byref(d), _ptr(U_canon), _ptr(psi_canon), _ptr(out_canon),
                                     1 if dagger else 0, prec, recon))
 
 
-def dw_apply_multi(g, kappa, U, clover, src, dst, nrhs, prec=F64, recon=RECON_18, dagger=False, stream=None):
+def dw_apply_multi(g, kappa, U, clover, src, dst, nrhs, prec=F64, recon=RECON_18, dagger=False, stream=None, mu=0.0):
     """D (or D^+) on nrhs spinor fields stored back to back in src / dst."""
-    d = _dirac(kappa)
+    d = _dirac(kappa, mu=mu)
     _check(lib().lqcd_dw_apply_multi(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(src), _ptr(dst), int(nrhs),
                                      1 if dagger else 0, prec, recon, _stream(stream)))
 

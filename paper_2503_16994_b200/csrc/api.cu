@@ -342,7 +342,7 @@ template <typename T>
 static cudaError_t dw_apply_t(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
                               void* out, bool dagger, int recon, cudaStream_t s) {
   Op<T> M;
-  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.recon = recon; M.eo = false;
+  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.mu = d->mu; M.recon = recon; M.eo = false;
   return M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s);
 }
 
@@ -350,7 +350,7 @@ template <typename T>
 static cudaError_t dw_multi_t(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
                               void* out, int nrhs, bool dagger, int recon, cudaStream_t s) {
   Op<T> M;
-  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.recon = recon; M.eo = false;
+  M.geom = h; M.U = U; M.A = clover; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.mu = d->mu; M.recon = recon; M.eo = false;
   return M.apply_multi(in, out, nrhs, dagger, s);
 }
 
@@ -401,6 +401,7 @@ lqcd_status lqcd_dw_eo_apply(const lqcd_geom* h, const lqcd_dirac* d, const void
   REQUIRE(h && d && U && clover && clover_inv && in_e && out_e && tmp, "lqcd_dw_eo_apply: NULL argument");
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_eo_apply: bad precision / recon");
   REQUIRE(out_e != in_e && tmp != in_e && tmp != out_e, "lqcd_dw_eo_apply: aliased buffers");
+  REQUIRE(d->mu == 0.0, "lqcd_dw_eo_apply: the even-odd operator does not support a twisted mass (mu != 0)");
   CUDA_TRY(DISPATCH_PREC(prec, dw_eo_t<double>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream)),
                          dw_eo_t<float>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream))),
            "dw_eo kernel");
@@ -486,6 +487,7 @@ Op<T> make_op(const SolveCtx& c, void* tmp) {
   M.Ainv = f64 ? c.f->clover_inv64 : c.f->clover_inv32;
   M.tmp = tmp;
   M.kappa = c.d->kappa;
+  M.mu = c.d->mu;
   M.recon = c.recon;
   M.eo = c.parm->eo != 0;
   return M;
@@ -559,6 +561,7 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
   REQUIRE(x != b, "lqcd_cg_solve: x aliases b");
   REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve: bad tol / maxiter");
   if (parm->eo) REQUIRE(f->clover64 && f->clover_inv64, "lqcd_cg_solve: eo needs clover64 and clover_inv64");
+  if (parm->eo) REQUIRE(d->mu == 0.0, "lqcd_cg_solve: the even-odd solver does not support a twisted mass (mu != 0)");
   if (parm->mixed) {
     REQUIRE(f->U32, "lqcd_cg_solve: mixed needs U32");
     REQUIRE((f->clover64 == nullptr) == (f->clover32 == nullptr), "lqcd_cg_solve: mixed needs clover32 iff clover64");

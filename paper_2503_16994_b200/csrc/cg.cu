@@ -28,7 +28,7 @@ cudaError_t Op<T>::apply(const void* in, void* out, bool dagger, int epi, void* 
   a.partial = partial;
   a.skip = skip;
   a.has_theta = geom->has_theta;
-  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  for (int d = 0; d < 4; d++) a.theta[d] = cx<T>((T)geom->th_re[d], (T)geom->th_im[d]);
   a.dagger = dagger ? 1 : 0;
   if (!eo) {
     a.A = (const T2<T>*)A;
@@ -36,6 +36,7 @@ cudaError_t Op<T>::apply(const void* in, void* out, bool dagger, int epi, void* 
     a.self = (const T2<T>*)in;
     a.out = (T2<T>*)out;
     a.k = (T)kappa;
+    a.tm = (T)(2.0 * kappa * (dagger ? -mu : mu));
     a.parity = -1;
     a.epi = epi;
     return launch_dw<T>(geom->g, a, recon, A ? DIAG_PRE : DIAG_ONE, s);
@@ -69,8 +70,9 @@ cudaError_t Op<T>::apply_multi(const void* in, void* out, int nrhs, bool dagger,
   a.self = (const T2<T>*)in;
   a.out = (T2<T>*)out;
   a.k = (T)kappa;
+  a.tm = (T)(2.0 * kappa * (dagger ? -mu : mu));
   a.has_theta = geom->has_theta;
-  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  for (int d = 0; d < 4; d++) a.theta[d] = cx<T>((T)geom->th_re[d], (T)geom->th_im[d]);
   a.dagger = dagger ? 1 : 0;
   a.parity = -1;
   a.epi = EPI_STORE;
@@ -90,7 +92,7 @@ cudaError_t Op<T>::hop_xpay(const void* in, const void* self, void* out, double 
   a.out = (T2<T>*)out;
   a.k = (T)k;
   a.has_theta = geom->has_theta;
-  for (int mu = 0; mu < 4; mu++) a.theta[mu] = cx<T>((T)geom->th_re[mu], (T)geom->th_im[mu]);
+  for (int d = 0; d < 4; d++) a.theta[d] = cx<T>((T)geom->th_re[d], (T)geom->th_im[d]);
   a.parity = parity;
   a.epi = EPI_STORE;
   return launch_dw<T>(geom->g, a, recon, DIAG_ONE, s);

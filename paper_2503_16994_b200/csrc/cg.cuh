@@ -12,6 +12,7 @@ struct Op {
   const void* Ainv;   // even-odd only
   void* tmp;          // even-odd only: one full spinor field (its odd half is used)
   double kappa;
+  double mu = 0.0;    // twisted mass (full operator only)
   int recon;
   bool eo;
   size_t ncomplex() const { return (size_t)(eo ? 1 : 2) * geom->g.Vh * 12; }

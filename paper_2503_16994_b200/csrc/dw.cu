@@ -141,6 +141,16 @@ __device__ __forceinline__ void clover_mul(const T2<T>* __restrict__ A, const in
 
 // One thread per site, one tile (both parities for the full operator) per CTA at a time; CTA b works through
 // tiles b, b + gridDim.x, ... (gridDim.x == ntiles gives the plain one-tile-per-CTA launch).
+// twisted mass (NEXT-4): o += i t gamma5 v, gamma5 = diag(1,1,-1,-1) in the chiral basis (components 0..5 / 6..11)
+template <typename T, int C0, int C1>
+__device__ __forceinline__ void add_twist(const T t, const cx<T> (&v)[12], cx<T> (&o)[12]) {
+#pragma unroll
+  for (int c = C0; c < C1; c++) {
+    const T tc = (c < 6) ? t : -t;
+    o[c] = cx<T>(fma(-tc, v[c].im, o[c].re), fma(tc, v[c].re, o[c].im));
+  }
+}
+
 template <typename T, int RECON, int DIAG, bool SPLIT>
 __device__ __forceinline__ void dw_body(const Geom& g, const DwArgs<T>& a) {
   constexpr int NCU = (RECON == 12) ? 6 : 9;
@@ -256,6 +266,7 @@ __device__ __forceinline__ void dw_body(const Geom& g, const DwArgs<T>& a) {
 #pragma unroll
             for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, v[c].re), fma(-a.k, acc[c].im, v[c].im));
           }
+          if (a.tm != T(0)) add_twist<T, 0, 12>(a.tm, v, res);
         }
       }
       // epilogue
@@ -654,6 +665,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             T2<T> w = sv[c * TV];
             v[c] = cx<T>(s * w.x, s * w.y);
           }
+          if (a.tm != T(0)) add_twist<T, 0, 6>(a.tm, v, acc);   // acc carries -(1/k) (A + i tm gamma5) psi
         }
         CloverPipe<T, NCU, 0, NSTC / 2>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
       }
@@ -668,6 +680,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             T2<T> w = sv[c * TV];
             v[c] = cx<T>(s * w.x, s * w.y);
           }
+          if (a.tm != T(0)) add_twist<T, 6, 12>(a.tm, v, acc);
         } else {
 #pragma unroll
           for (int c = 0; c < 12; c++) {
@@ -687,6 +700,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       } else if (live) {
 #pragma unroll
         for (int c = 0; c < 12; c++) res[c] = cx<T>(fma(-a.k, acc[c].re, v[c].re), fma(-a.k, acc[c].im, v[c].im));
+        if (a.tm != T(0)) add_twist<T, 0, 12>(a.tm, v, res);
       }
       if (!live) {
 #pragma unroll

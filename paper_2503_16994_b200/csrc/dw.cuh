@@ -19,6 +19,8 @@ struct DwArgs {
   double* partial;                     // one partial sum per CTA
   const int* skip;                     // device flag: if non-NULL and *skip != 0 the kernel does nothing
   T k;                                 // kappa (or kappa^2 for the even-odd operator)
+  T tm;                                // twisted mass term: + i tm gamma5 self added to the result (2 kappa mu; -2 kappa mu
+                                       // for D^+); 0 = absent.  Full-lattice operator only.
   cx<T> theta[4];
   int has_theta;
   int dagger;
