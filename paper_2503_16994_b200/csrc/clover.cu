@@ -7,234 +7,297 @@
 // i.e. with the Hermitian 3x3 matrices G_k = i(+-E_k - B_k) each chiral block is
 //   1 + kappa csw [[G_3, G_1 - i G_2], [G_1 + i G_2, -G_3]]          (row index 3*s + a)
 // stored packed (6 real diagonal entries + 15 complex below the diagonal).  Always evaluated in fp64
-// (R14); the result is rounded once to the requested precision.  One thread per site.
+// (R14); the result is rounded once to the requested precision.
 #include "kernels.cuh"
 
 namespace lqcd {
 
+// Kernel structure: one thread per site.  The six Hermitian matrices i F^_{mu nu} are computed one plane at a time
+// in a rolled loop (4 leaves x 3 SU(3) products per plane, leaf loop rolled too) and parked in shared memory
+// as 9 reals each (54 doubles per thread, [component][thread]: conflict-free); the two chiral blocks are then
+// assembled entry by entry straight into the packed output, so no 6x6 array is ever live unless the inverse is
+// requested.  Arithmetic bound: 72 products x 198 flop = 14.3 kflop fp64 per site against 1152 bytes moved.
+
 struct m3 { double2 e[3][3]; };
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a*conj(b)
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 s) {  // s + a*b
+  return make_double2(fma(a.x, b.x, fma(-a.y, b.y, s.x)), fma(a.x, b.y, fma(a.y, b.x, s.y)));
+}
 
-__device__ m3 mmul(const m3& a, const m3& b) {
+// c = a b
+__device__ __forceinline__ m3 mul_nn(const m3& a, const m3& b) {
   m3 c;
+#pragma unroll
   for (int i = 0; i < 3; i++)
-    for (int j = 0; j < 3; j++) {
-      double2 s = cmul(a.e[i][0], b.e[0][j]);
-      s = cadd(s, cmul(a.e[i][1], b.e[1][j]));
-      s = cadd(s, cmul(a.e[i][2], b.e[2][j]));
-      c.e[i][j] = s;
-    }
+#pragma unroll
+    for (int j = 0; j < 3; j++) c.e[i][j] = cfma(a.e[i][2], b.e[2][j], cfma(a.e[i][1], b.e[1][j], cmul(a.e[i][0], b.e[0][j])));
   return c;
 }
-__device__ m3 mdag(const m3& a) {
-  m3 c;
+// q += a b
+__device__ __forceinline__ void acc_nn(m3& q, const m3& a, const m3& b) {
+#pragma unroll
   for (int i = 0; i < 3; i++)
-    for (int j = 0; j < 3; j++) c.e[i][j] = make_double2(a.e[j][i].x, -a.e[j][i].y);
-  return c;
+#pragma unroll
+    for (int j = 0; j < 3; j++) q.e[i][j] = cfma(a.e[i][2], b.e[2][j], cfma(a.e[i][1], b.e[1][j], cfma(a.e[i][0], b.e[0][j], q.e[i][j])));
 }
 
 struct CloverCtx {
   Geom g;
   const double2* U;
-  int recon;
   double phiT[3];
 };
 
-// U_mu at the point x (coordinates may be one or two steps outside the box).
-// Spatial directions wrap; time wraps for periodic BC; SF: slice x4 = L4 is the fixed boundary field W' (D7).
-__device__ m3 link_at(const CloverCtx& c, const int xin[4], int mu) {
+// The site a thread works on: tile, local coordinates, parity, global time coordinate.
+struct SitePos {
+  int tile, par, x3;
+  int l[4];
+};
+
+// W = U_dir (dag == 0) or U_dir^+ (dag != 0) at the point x + dm mu^ + dn nu^ (|dm|, |dn| <= 1).
+// The neighbour is found from the local coordinates: a step out of the tile follows the neighbour-tile table
+// (periodic in every direction), so no division by a run-time extent is needed.  SF: the slice x4 = L4 is the
+// fixed boundary field W' (D7) and is never read from memory.
+// mu, nu, dir are run-time values: coordinates are shifted by comparison, never by indexing a register array.
+template <int RECON>
+__device__ __forceinline__ m3 link_at(const CloverCtx& c, const SitePos& sp, int mu, int dm, int nu, int dn, int dir, int dag) {
   const Geom& g = c.g;
-  int x[4];
-  for (int i = 0; i < 3; i++) {
-    x[i] = xin[i];
-    if (x[i] < 0) x[i] += g.L[i];
-    if (x[i] >= g.L[i]) x[i] -= g.L[i];
-  }
-  x[3] = xin[3];
+  constexpr int NCU = RECON == 12 ? 6 : 9;
   m3 r;
   const bool sf = (g.bc == LQCD_BC_SF_ORBI || g.bc == LQCD_BC_SF_AFWB);
-  if (sf && x[3] == g.L[3]) {
+  const int x3 = sp.x3 + (mu == 3 ? dm : 0) + (nu == 3 ? dn : 0);
+  if (sf && x3 == g.L[3]) {   // diagonal: its own transpose; dagger = conjugate
+#pragma unroll
     for (int i = 0; i < 3; i++)
+#pragma unroll
       for (int j = 0; j < 3; j++) r.e[i][j] = make_double2(0.0, 0.0);
-    if (mu < 3)
+    if (dir < 3) {
+      const int Ld = dir == 0 ? g.L[0] : (dir == 1 ? g.L[1] : g.L[2]);
+#pragma unroll
       for (int i = 0; i < 3; i++) {
         double s, co;
-        sincos(c.phiT[i] / g.L[mu], &s, &co);
-        r.e[i][i] = make_double2(co, s);
+        sincos(c.phiT[i] / Ld, &s, &co);
+        r.e[i][i] = make_double2(co, dag ? -s : s);
       }
+    }
     return r;
   }
-  if (x[3] < 0) x[3] += g.L[3];
-  if (x[3] >= g.L[3]) x[3] -= g.L[3];
-  int p, tile, j;
-  site_locate(g, x, p, tile, j);
-  const int NCU = c.recon == 12 ? 6 : 9;
-  for (int k = 0; k < NCU; k++) r.e[k / 3][k % 3] = __ldg(c.U + field_offset(g, 4 * NCU, p, tile, mu * NCU + k, j));
-  if (c.recon == 12) {
-    for (int k = 0; k < 3; k++) {
-      int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
-      double2 v = csub(cmul(r.e[0][k1], r.e[1][k2]), cmul(r.e[0][k2], r.e[1][k1]));
-      r.e[2][k] = make_double2(v.x, -v.y);
+  int l[4];
+  int t = sp.tile;
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    l[i] = sp.l[i] + (i == mu ? dm : 0) + (i == nu ? dn : 0);
+    if (l[i] < 0) {
+      l[i] += g.b[i];
+      t = __ldg(g.tile_tab + (size_t)t * TILE_TAB + 2 * i + 1);
+    } else if (l[i] >= g.b[i]) {
+      l[i] -= g.b[i];
+      t = __ldg(g.tile_tab + (size_t)t * TILE_TAB + 2 * i);
     }
   }
+  const int p = (sp.par + dm + dn) & 1;
+  const double2* up = c.U + field_offset(g, 4 * NCU, p, t, dir * NCU, local_index(g, l));
+  m3 u;
+#pragma unroll
+  for (int k = 0; k < NCU; k++) u.e[k / 3][k % 3] = __ldg(up + (size_t)k * g.TV);
+  if (RECON == 12) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+      const int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
+      double2 v = csub(cmul(u.e[0][k1], u.e[1][k2]), cmul(u.e[0][k2], u.e[1][k1]));
+      u.e[2][k] = make_double2(v.x, -v.y);
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) r.e[i][j] = dag ? make_double2(u.e[j][i].x, -u.e[j][i].y) : u.e[i][j];
   return r;
 }
 
-__device__ __forceinline__ void shifted(const int x[4], int mu, int d, int y[4]) {
-  for (int i = 0; i < 4; i++) y[i] = x[i];
-  y[mu] += d;
-}
+// The four leaves of Q_{mu nu}(x), each a closed path of four oriented links starting and ending at x:
+// per link (dm, dn, direction: 0 = mu / 1 = nu, dagger)
+//   1: U_mu(x) U_nu(x+mu) U_mu(x+nu)^+ U_nu(x)^+
+//   2: U_nu(x) U_mu(x-mu+nu)^+ U_nu(x-mu)^+ U_mu(x-mu)
+//   3: U_mu(x-mu)^+ U_nu(x-mu-nu)^+ U_mu(x-mu-nu) U_nu(x-nu)
+//   4: U_nu(x-nu)^+ U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^+
+__constant__ signed char LEAF[4][4][4] = {
+    {{0, 0, 0, 0}, {+1, 0, 1, 0}, {0, +1, 0, 1}, {0, 0, 1, 1}},
+    {{0, 0, 1, 0}, {-1, +1, 0, 1}, {-1, 0, 1, 1}, {-1, 0, 0, 0}},
+    {{-1, 0, 0, 1}, {-1, -1, 1, 1}, {-1, -1, 0, 0}, {0, -1, 1, 0}},
+    {{0, -1, 1, 1}, {0, -1, 0, 0}, {+1, -1, 1, 0}, {0, 0, 0, 1}},
+};
 
-// i * F^_{mu nu}(x)  (Hermitian)
-__device__ m3 i_fhat(const CloverCtx& c, const int x[4], int mu, int nu) {
-  int xpm[4], xpn[4], xmm[4], xmn[4], xmmpn[4], xmmmn[4], xpmmn[4];
-  shifted(x, mu, +1, xpm);
-  shifted(x, nu, +1, xpn);
-  shifted(x, mu, -1, xmm);
-  shifted(x, nu, -1, xmn);
-  shifted(xmm, nu, +1, xmmpn);
-  shifted(xmm, nu, -1, xmmmn);
-  shifted(xpm, nu, -1, xpmmn);
+// i * F^_{mu nu}(x)  (Hermitian), as 9 reals: diagonal, then (re, im) of [1][0], [2][0], [2][1].
+// The leaf loop stays rolled (3 products + 4 link fetches of code): the unrolled body does not fit the
+// instruction cache and the kernel then stalls on instruction fetch.
+template <int RECON>
+__device__ __forceinline__ void i_fhat(const CloverCtx& c, const SitePos& sp, int mu, int nu, double (&h)[9]) {
   m3 Q;
-  {  // U_mu(x) U_nu(x+mu) U_mu(x+nu)^+ U_nu(x)^+
-    m3 a = mmul(link_at(c, x, mu), link_at(c, xpm, nu));
-    m3 b = mmul(link_at(c, x, nu), link_at(c, xpn, mu));
-    Q = mmul(a, mdag(b));
-  }
-  {  // U_nu(x) U_mu(x-mu+nu)^+ U_nu(x-mu)^+ U_mu(x-mu)
-    m3 a = mmul(link_at(c, x, nu), mdag(link_at(c, xmmpn, mu)));
-    m3 b = mmul(mdag(link_at(c, xmm, nu)), link_at(c, xmm, mu));
-    m3 l = mmul(a, b);
-    for (int i = 0; i < 3; i++)
-      for (int j = 0; j < 3; j++) Q.e[i][j] = cadd(Q.e[i][j], l.e[i][j]);
-  }
-  {  // U_mu(x-mu)^+ U_nu(x-mu-nu)^+ U_mu(x-mu-nu) U_nu(x-nu)
-    m3 a = mmul(link_at(c, xmmmn, nu), link_at(c, xmm, mu));
-    m3 b = mmul(link_at(c, xmmmn, mu), link_at(c, xmn, nu));
-    m3 l = mmul(mdag(a), b);
-    for (int i = 0; i < 3; i++)
-      for (int j = 0; j < 3; j++) Q.e[i][j] = cadd(Q.e[i][j], l.e[i][j]);
-  }
-  {  // U_nu(x-nu)^+ U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^+
-    m3 a = mmul(mdag(link_at(c, xmn, nu)), link_at(c, xmn, mu));
-    m3 b = mmul(link_at(c, xpmmn, nu), mdag(link_at(c, x, mu)));
-    m3 l = mmul(a, b);
-    for (int i = 0; i < 3; i++)
-      for (int j = 0; j < 3; j++) Q.e[i][j] = cadd(Q.e[i][j], l.e[i][j]);
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) Q.e[i][j] = make_double2(0.0, 0.0);
+#pragma unroll 1
+  for (int lf = 0; lf < 4; lf++) {
+#define LQCD_W(s) link_at<RECON>(c, sp, mu, LEAF[lf][s][0], nu, LEAF[lf][s][1], LEAF[lf][s][2] ? nu : mu, LEAF[lf][s][3])
+    m3 t = mul_nn(LQCD_W(0), LQCD_W(1));
+    m3 t2 = mul_nn(t, LQCD_W(2));
+    acc_nn(Q, t2, LQCD_W(3));
+#undef LQCD_W
   }
   // i (Q - Q^+)/8 :  (Q - Q^+)_{ij} = Q_ij - conj(Q_ji) ;  i*(a + ib) = -b + ia
-  m3 F;
-  for (int i = 0; i < 3; i++)
-    for (int j = 0; j < 3; j++) {
-      double re = (Q.e[i][j].x - Q.e[j][i].x) * 0.125;
-      double im = (Q.e[i][j].y + Q.e[j][i].y) * 0.125;
-      F.e[i][j] = make_double2(-im, re);
-    }
-  return F;
+#pragma unroll
+  for (int i = 0; i < 3; i++) h[i] = -0.25 * Q.e[i][i].y;
+  h[3] = -(Q.e[1][0].y + Q.e[0][1].y) * 0.125;  h[4] = (Q.e[1][0].x - Q.e[0][1].x) * 0.125;
+  h[5] = -(Q.e[2][0].y + Q.e[0][2].y) * 0.125;  h[6] = (Q.e[2][0].x - Q.e[0][2].x) * 0.125;
+  h[7] = -(Q.e[2][1].y + Q.e[1][2].y) * 0.125;  h[8] = (Q.e[2][1].x - Q.e[1][2].x) * 0.125;
+}
+
+// element (a, b) of a Hermitian 3x3 held as 9 reals (layout of i_fhat)
+__device__ __forceinline__ double2 herm_at(const double (&h)[9], int a, int b) {
+  if (a == b) return make_double2(h[a], 0.0);
+  const int hi = a > b ? a : b, lo = a > b ? b : a;
+  const int o = 3 + 2 * (hi * (hi - 1) / 2 + lo);
+  return make_double2(h[o], a > b ? h[o + 1] : -h[o + 1]);
 }
 
 // in-place inverse of a Hermitian positive-definite 6x6 (Gauss-Jordan, no pivoting needed for HPD)
-__device__ void invert6(double2 (&a)[6][6]) {
+__device__ __forceinline__ void invert6(double2 (&a)[6][6]) {
+#pragma unroll
   for (int c = 0; c < 6; c++) {
-    double piv = 1.0 / a[c][c].x;  // diagonal of an HPD Schur complement is real
+    const double piv = 1.0 / a[c][c].x;  // diagonal of an HPD Schur complement is real
     a[c][c] = make_double2(1.0, 0.0);
+#pragma unroll
     for (int j = 0; j < 6; j++) a[c][j] = make_double2(a[c][j].x * piv, a[c][j].y * piv);
+#pragma unroll
     for (int r = 0; r < 6; r++) {
       if (r == c) continue;
-      double2 f = a[r][c];
+      const double2 f = a[r][c];
       a[r][c] = make_double2(0.0, 0.0);
+#pragma unroll
       for (int j = 0; j < 6; j++) a[r][j] = csub(a[r][j], cmul(f, a[c][j]));
     }
   }
 }
 
 template <typename T>
-__device__ void store_packed(const Geom& g, typename vec2<T>::type* out, int p, int tile, int j, int ch, const double2 (&a)[6][6]) {
+__device__ __forceinline__ void store_packed(typename vec2<T>::type* out, size_t TV, const double2 (&a)[6][6]) {
+#pragma unroll
   for (int k = 0; k < 3; k++) {
     typename vec2<T>::type d;
     d.x = (T)a[2 * k][2 * k].x;
     d.y = (T)a[2 * k + 1][2 * k + 1].x;
-    out[field_offset(g, 36, p, tile, 18 * ch + k, j)] = d;
+    out[k * TV] = d;
   }
+#pragma unroll
   for (int i = 1; i < 6; i++)
+#pragma unroll
     for (int jj = 0; jj < i; jj++) {
       typename vec2<T>::type l;
       l.x = (T)a[i][jj].x;
       l.y = (T)a[i][jj].y;
-      out[field_offset(g, 36, p, tile, 18 * ch + 3 + i * (i - 1) / 2 + jj, j)] = l;
+      out[(3 + i * (i - 1) / 2 + jj) * TV] = l;
     }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(128) clover_kernel(const CloverCtx c, const CloverParm cp, typename vec2<T>::type* A,
-                                                     typename vec2<T>::type* Ainv) {
+constexpr int CLV_THREADS = 128;
+#ifndef CLV_MINB
+#define CLV_MINB 3
+#endif
+
+template <typename T, int RECON, bool INV>
+__global__ void __launch_bounds__(CLV_THREADS, CLV_MINB) clover_kernel(const CloverCtx c, const CloverParm cp, typename vec2<T>::type* A,
+                                                             typename vec2<T>::type* Ainv) {
+  extern __shared__ double sF[];   // [6 planes][9][CLV_THREADS]
   const Geom& g = c.g;
   long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 2 * g.Vh) return;
-  // thread -> site in internal order (stores are coalesced over j)
-  int p = (int)(idx / g.Vh);
-  long long rem = idx - (long long)p * g.Vh;
-  int tile = (int)(rem / g.TV);
-  int j = (int)(rem - (long long)tile * g.TV);
-  int Tc[4], l[4], x[4];
-  tile_coords(g, tile, Tc);
-  local_coords(g, j, p, l);
-  for (int i = 0; i < 4; i++) x[i] = Tc[i] * g.b[i] + l[i];
+  // thread -> site: a CTA takes runs of JC = min(64, TV) consecutive checkerboard indices of BOTH parities of a
+  // tile (for 4^4 tiles: a 4x4x4x2 slab), so that the links a site shares with its neighbours are fetched by
+  // the same CTA at the same time and hit in L1; stores stay coalesced over j in runs of JC.
+  const int JC = g.TV < 64 ? g.TV : 64;
+  const long long unit = idx / (2 * JC);
+  const int r = (int)(idx - unit * (2 * JC));
+  const int cpt = g.TV / JC;   // runs per tile
+  const int tile = (int)(unit / cpt);
+  const int p = r / JC;
+  const int j = (int)(unit - (long long)tile * cpt) * JC + (r - p * JC);
+  SitePos sp;
+  sp.tile = tile;
+  sp.par = p;
+  local_coords(g, j, p, sp.l);
+  sp.x3 = __ldg(g.tile_tab + (size_t)tile * TILE_TAB + 8) + sp.l[3];
+  const int x3 = sp.x3;
 
-  double2 blk[2][6][6];
-  for (int ch = 0; ch < 2; ch++)
-    for (int i = 0; i < 6; i++)
-      for (int k = 0; k < 6; k++) blk[ch][i][k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
-
-  const bool fz = (g.bc != LQCD_BC_PERIODIC) && frozen_slice(g, x[3]);
-  if (!fz) {
-    const double cc = cp.kappa * cp.csw;
-    if (cc != 0.0) {
-      for (int k = 0; k < 3; k++) {
-        const int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
-        m3 E = i_fhat(c, x, k, 3);    // i E_k = i F^_{k4}
-        m3 B = i_fhat(c, x, k1, k2);  // i B_k = i F^_{k1 k2}  (23, 31, 12)
-        for (int ch = 0; ch < 2; ch++) {
-          const double se = (ch == 0) ? 1.0 : -1.0;
-          for (int a = 0; a < 3; a++)
-            for (int b = 0; b < 3; b++) {
-              // G = i(+-E - B)
-              double2 G = make_double2(se * E.e[a][b].x - B.e[a][b].x, se * E.e[a][b].y - B.e[a][b].y);
-              G.x *= cc; G.y *= cc;
-              if (k == 2) {  // sigma_3: +G on (0,0), -G on (1,1)
-                blk[ch][a][b] = cadd(blk[ch][a][b], G);
-                blk[ch][3 + a][3 + b] = csub(blk[ch][3 + a][3 + b], G);
-              } else if (k == 0) {  // sigma_1: G on (0,1) and (1,0)
-                blk[ch][a][3 + b] = cadd(blk[ch][a][3 + b], G);
-                blk[ch][3 + a][b] = cadd(blk[ch][3 + a][b], G);
-              } else {  // sigma_2: -i G on (0,1), +i G on (1,0)
-                blk[ch][a][3 + b] = cadd(blk[ch][a][3 + b], make_double2(G.y, -G.x));
-                blk[ch][3 + a][b] = cadd(blk[ch][3 + a][b], make_double2(-G.y, G.x));
-              }
-            }
-        }
+  const bool fz = (g.bc != LQCD_BC_PERIODIC) && frozen_slice(g, x3);
+  const double cc = cp.kappa * cp.csw;
+  const bool have_f = !fz && cc != 0.0;
+  double* myF = sF + threadIdx.x;
+  if (have_f) {
+    // planes 0..2: E_k = F^_{k4};  planes 3..5: B_k = F^_{k1 k2} = (23, 31, 12)
+#pragma unroll 1
+    for (int pl = 0; pl < 6; pl++) {
+      const int k = pl < 3 ? pl : pl - 3;
+      const int mu = pl < 3 ? k : (k + 1) % 3;
+      const int nu = pl < 3 ? 3 : (k + 2) % 3;
+      double h[9];
+      i_fhat<RECON>(c, sp, mu, nu, h);
+#pragma unroll
+      for (int r = 0; r < 9; r++) myF[(pl * 9 + r) * CLV_THREADS] = h[r];
+    }
+  }
+  double dadd = 0.0;
+  if (!fz && g.bc != LQCD_BC_PERIODIC && cp.ct != 1.0) {  // R10: + 2 kappa (ct - 1) next to the frozen slices
+    const int last = (g.bc == LQCD_BC_OPEN) ? g.L[3] - 2 : g.L[3] - 1;
+    if (x3 == 1) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
+    if (x3 == last) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
+  }
+  const size_t TV = g.TV;
+#pragma unroll 1
+  for (int ch = 0; ch < 2; ch++) {
+    // G_k = i(+-E_k - B_k), scaled by kappa csw
+    double G[3][9];
+    const double se = (ch == 0) ? cc : -cc;
+#pragma unroll
+    for (int k = 0; k < 3; k++)
+#pragma unroll
+      for (int r = 0; r < 9; r++)
+        G[k][r] = have_f ? se * myF[(k * 9 + r) * CLV_THREADS] - cc * myF[((3 + k) * 9 + r) * CLV_THREADS] : 0.0;
+    // block = 1 + [[G_3, G_1 - i G_2], [G_1 + i G_2, -G_3]]   (row index 3*s + a)
+    double2 blk[6][6];
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        const double2 g1 = herm_at(G[0], a, b), g2 = herm_at(G[1], a, b), g3 = herm_at(G[2], a, b);
+        const double one = (a == b) ? 1.0 + dadd : 0.0;
+        blk[a][b] = make_double2(one + g3.x, g3.y);
+        blk[3 + a][3 + b] = make_double2(one - g3.x, -g3.y);
+        blk[a][3 + b] = make_double2(g1.x + g2.y, g1.y - g2.x);
+        blk[3 + a][b] = make_double2(g1.x - g2.y, g1.y + g2.x);
       }
-    }
-    if (g.bc != LQCD_BC_PERIODIC && cp.ct != 1.0) {  // R10: + 2 kappa (ct - 1) next to the frozen slices
-      const int last = (g.bc == LQCD_BC_OPEN) ? g.L[3] - 2 : g.L[3] - 1;
-      double add = 0.0;
-      if (x[3] == 1) add += 2.0 * cp.kappa * (cp.ct - 1.0);
-      if (x[3] == last) add += 2.0 * cp.kappa * (cp.ct - 1.0);
-      for (int ch = 0; ch < 2; ch++)
-        for (int i = 0; i < 6; i++) blk[ch][i][i].x += add;
+    const size_t off = field_offset(g, 36, p, tile, 18 * ch, j);
+    store_packed<T>(A + off, TV, blk);
+    if (INV) {
+      invert6(blk);
+      store_packed<T>(Ainv + off, TV, blk);
     }
   }
-  for (int ch = 0; ch < 2; ch++) store_packed<T>(g, A, p, tile, j, ch, blk[ch]);
-  if (Ainv) {
-    for (int ch = 0; ch < 2; ch++) {
-      invert6(blk[ch]);
-      store_packed<T>(g, Ainv, p, tile, j, ch, blk[ch]);
-    }
-  }
+}
+
+template <typename T, int RECON, bool INV>
+static cudaError_t clover_launch(const CloverCtx& c, const CloverParm& cp, void* clover, void* clover_inv, cudaStream_t s) {
+  typedef typename vec2<T>::type T2;
+  const size_t smem = (size_t)54 * CLV_THREADS * sizeof(double);
+  cudaError_t e = cudaFuncSetAttribute(clover_kernel<T, RECON, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  unsigned blocks = (unsigned)((2 * c.g.Vh + CLV_THREADS - 1) / CLV_THREADS);
+  clover_kernel<T, RECON, INV><<<blocks, CLV_THREADS, smem, s>>>(c, cp, (T2*)clover, (T2*)clover_inv);
+  count_launch();
+  return cudaGetLastError();
 }
 
 cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, int recon, void* clover, void* clover_inv,
@@ -242,15 +305,17 @@ cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, i
   CloverCtx c;
   c.g = g;
   c.U = (const double2*)U64;
-  c.recon = recon;
   for (int i = 0; i < 3; i++) c.phiT[i] = cp.phiT[i];
-  unsigned blocks = (unsigned)((2 * g.Vh + 127) / 128);
-  if (out_prec == LQCD_F64)
-    clover_kernel<double><<<blocks, 128, 0, s>>>(c, cp, (double2*)clover, (double2*)clover_inv);
-  else
-    clover_kernel<float><<<blocks, 128, 0, s>>>(c, cp, (float2*)clover, (float2*)clover_inv);
-  count_launch();
-  return cudaGetLastError();
+  const bool f64 = out_prec == LQCD_F64, r12 = recon == 12, inv = clover_inv != nullptr;
+#define LQCD_CLV(T, R, I) return clover_launch<T, R, I>(c, cp, clover, clover_inv, s)
+  if (f64) {
+    if (r12) { if (inv) LQCD_CLV(double, 12, true); else LQCD_CLV(double, 12, false); }
+    else     { if (inv) LQCD_CLV(double, 18, true); else LQCD_CLV(double, 18, false); }
+  } else {
+    if (r12) { if (inv) LQCD_CLV(float, 12, true); else LQCD_CLV(float, 12, false); }
+    else     { if (inv) LQCD_CLV(float, 18, true); else LQCD_CLV(float, 18, false); }
+  }
+#undef LQCD_CLV
 }
 
 }  // namespace lqcd
