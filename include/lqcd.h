@@ -47,10 +47,16 @@ typedef enum {
   LQCD_EUNSUPPORTED = -6
 } lqcd_status;
 
-typedef enum { LQCD_BC_PERIODIC = 0, LQCD_BC_OPEN = 1, LQCD_BC_SF_ORBI = 2, LQCD_BC_SF_AFWB = 3 } lqcd_bc;
+typedef enum {
+  LQCD_BC_PERIODIC = 0, LQCD_BC_OPEN = 1, LQCD_BC_SF_ORBI = 2, LQCD_BC_SF_AFWB = 3,
+  LQCD_BC_SLAB = 4   /* one time slab of a lattice periodic in time: see "Time-direction domain decomposition" below */
+} lqcd_bc;
 typedef enum { LQCD_F64 = 0, LQCD_F32 = 1 } lqcd_prec;
 typedef enum { LQCD_RECON_18 = 18, LQCD_RECON_12 = 12 } lqcd_recon;
-typedef enum { LQCD_FIELD_GAUGE = 0, LQCD_FIELD_SPINOR = 1, LQCD_FIELD_CLOVER = 2, LQCD_FIELD_WORKSPACE = 3 } lqcd_field_kind;
+typedef enum {
+  LQCD_FIELD_GAUGE = 0, LQCD_FIELD_SPINOR = 1, LQCD_FIELD_CLOVER = 2, LQCD_FIELD_WORKSPACE = 3,
+  LQCD_FIELD_FACE = 4   /* one half-spinor time face of a slab: 6 complex numbers x L[0] L[1] L[2] sites */
+} lqcd_field_kind;
 
 /* Geometry (the paper's SpaceParm, plus the fermion phases of DiracParam, :119). */
 typedef struct {
@@ -150,6 +156,29 @@ lqcd_status lqcd_correlator_ps(const lqcd_geom* g, const void* columns, int ncol
 lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host,
                                const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
                                lqcd_recon recon);
+
+/* Time-direction domain decomposition (the volume one GPU holds
+ * is the paper's stated limit).  A rank owns the slab x4 in [t0, t0 + L[3]) of a lattice periodic in time and creates
+ * its geometry with bc = LQCD_BC_SLAB, L[3] = the slab's extent and theta[3] = theta4 * L[3] / L4 (the per-link
+ * phase exp(i theta4 / L4) of the whole lattice; an antiperiodic lattice is theta4 = pi).  One application of D:
+ *   1. lqcd_dw_slab_pack   : in -> send_lo, send_hi (DEVICE, caller-owned, lqcd_field_bytes(LQCD_FIELD_FACE) each):
+ *                            half spinors of the first / last slice; the backward hop's link multiply is done here.
+ *   2. the caller moves send_lo to the rank below (its recv_hi) and send_hi to the rank above (its recv_lo); with one
+ *      rank the two are swapped in place, which reproduces the periodic lattice;
+ *   3. lqcd_dw_apply / lqcd_dwdag_apply on the slab (the hops through the two time faces are left out; it may run
+ *      while the faces travel);
+ *   4. lqcd_dw_slab_faces  : out -= kappa * (the two missing hops) from recv_lo, recv_hi.  Call after 3 on `out`.
+ * Step 3 + 4 equal the whole-lattice operator restricted to the slab (rounding order of the last additions aside).
+ * lqcd_clover_build_slab: Csw! on the slab; halo_lo / halo_hi = the time slice just below / above the slab, DEVICE,
+ * canonical fp64 layout [L0 L1 L2][4][3][3] (a one-off exchange per configuration).  On a SLAB geometry the solver,
+ * the even-odd operator and lqcd_clover_build return LQCD_EUNSUPPORTED (they would ignore the faces). */
+lqcd_status lqcd_dw_slab_pack(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* in, void* send_lo,
+                              void* send_hi, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream);
+lqcd_status lqcd_dw_slab_faces(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* recv_lo,
+                               const void* recv_hi, void* out, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream);
+lqcd_status lqcd_clover_build_slab(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, lqcd_recon recon,
+                                   const void* halo_lo, const void* halo_hi, void* clover, void* clover_inv,
+                                   lqcd_prec out_prec, void* stream);
 
 /* SURVEY.md 8(f) NEXT-1 (the 12 colour-spin sources of propagator! share one gauge field): D or D^+
  * (dagger != 0) applied to nrhs (1..64) spinor fields in one pass.  in / out: DEVICE arrays of nrhs internal spinor

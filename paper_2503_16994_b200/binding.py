@@ -12,10 +12,10 @@ LIB_PATH = os.path.join(HERE, "liblqcd_b200.so")
 
 # enums of include/lqcd.h
 OK, EINVAL, ENOMEM, ECUDA, ENOTCONV, EBREAKDOWN, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
-BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB = 0, 1, 2, 3
+BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB, BC_SLAB = 0, 1, 2, 3, 4
 F64, F32 = 0, 1
 RECON_18, RECON_12 = 18, 12
-FIELD_GAUGE, FIELD_SPINOR, FIELD_CLOVER, FIELD_WORKSPACE = 0, 1, 2, 3
+FIELD_GAUGE, FIELD_SPINOR, FIELD_CLOVER, FIELD_WORKSPACE, FIELD_FACE = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "lqcd_geom_create", "lqcd_geom_destroy", "lqcd_geom_info", "lqcd_field_bytes",
@@ -23,7 +23,8 @@ EXPORTS = [
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
-    "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps",
+    "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
+    "lqcd_clover_build_slab",
 ]
 
 
@@ -175,6 +176,26 @@ def clover_build(g, kappa, csw, U64, clover, clover_inv=None, recon=RECON_18, ou
     d = _dirac(kappa, csw, ct)
     _check(lib().lqcd_clover_build(g, ctypes.byref(d), _ptr(U64), recon, _ptr(clover), _ptr(clover_inv), out_prec,
                                    _stream(stream)))
+
+
+def clover_build_slab(g, kappa, csw, U64, halo_lo, halo_hi, clover, clover_inv=None, recon=RECON_18, out_prec=F64,
+                      stream=None):
+    """Csw! on a time slab (BC_SLAB); halo_lo / halo_hi: the neighbour ranks' adjacent time slices, canonical fp64."""
+    d = _dirac(kappa, csw)
+    _check(lib().lqcd_clover_build_slab(g, ctypes.byref(d), _ptr(U64), recon, _ptr(halo_lo), _ptr(halo_hi), _ptr(clover),
+                                        _ptr(clover_inv), out_prec, _stream(stream)))
+
+
+def dw_slab_pack(g, kappa, U, psi_in, send_lo, send_hi, dagger=False, prec=F64, recon=RECON_18, stream=None):
+    d = _dirac(kappa)
+    _check(lib().lqcd_dw_slab_pack(g, ctypes.byref(d), _ptr(U), _ptr(psi_in), _ptr(send_lo), _ptr(send_hi),
+                                   1 if dagger else 0, prec, recon, _stream(stream)))
+
+
+def dw_slab_faces(g, kappa, U, recv_lo, recv_hi, psi_out, dagger=False, prec=F64, recon=RECON_18, stream=None):
+    d = _dirac(kappa)
+    _check(lib().lqcd_dw_slab_faces(g, ctypes.byref(d), _ptr(U), _ptr(recv_lo), _ptr(recv_hi), _ptr(psi_out),
+                                    1 if dagger else 0, prec, recon, _stream(stream)))
 
 
 def dw_apply(g, kappa, U, clover, psi_in, psi_out, prec=F64, recon=RECON_18, stream=None, mu=0.0):

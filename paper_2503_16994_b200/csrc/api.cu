@@ -153,6 +153,13 @@ using namespace lqcd;
       return LQCD_EINVAL;           \
     }                               \
   } while (0)
+#define UNSUPPORTED_ON_SLAB(h, what)                                                                     \
+  do {                                                                                                   \
+    if ((h)->g.bc == LQCD_BC_SLAB) {                                                                     \
+      set_error("%s: not available on a LQCD_BC_SLAB geometry (the time faces would be ignored)", what); \
+      return LQCD_EUNSUPPORTED;                                                                          \
+    }                                                                                                    \
+  } while (0)
 #define CUDA_TRY(e, what)                        \
   do {                                           \
     if (!cuda_ok((e), what)) return LQCD_ECUDA;  \
@@ -187,10 +194,10 @@ lqcd_status lqcd_set_option(const char* key, const char* value) {
 lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   REQUIRE(desc && out, "lqcd_geom_create: NULL argument");
   *out = nullptr;
-  REQUIRE(desc->bc >= LQCD_BC_PERIODIC && desc->bc <= LQCD_BC_SF_AFWB, "lqcd_geom_create: bad bc %d", (int)desc->bc);
+  REQUIRE(desc->bc >= LQCD_BC_PERIODIC && desc->bc <= LQCD_BC_SLAB, "lqcd_geom_create: bad bc %d", (int)desc->bc);
   for (int i = 0; i < 4; i++)
     REQUIRE(desc->L[i] >= 2 && desc->L[i] % 2 == 0, "lqcd_geom_create: extent L[%d]=%d must be even and >= 2 (R13)", i, desc->L[i]);
-  if (desc->bc != LQCD_BC_PERIODIC) REQUIRE(desc->L[3] >= 4, "lqcd_geom_create: open/SF need L[3] >= 4");
+  if (desc->bc != LQCD_BC_PERIODIC) REQUIRE(desc->L[3] >= 4, "lqcd_geom_create: open/SF/slab need L[3] >= 4");
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     set_error("lqcd_geom_create: no CUDA device (this library has no CPU fallback)");
@@ -272,6 +279,7 @@ size_t lqcd_field_bytes(const lqcd_geom* h, lqcd_field_kind kind, lqcd_prec prec
     case LQCD_FIELD_GAUGE: return sites * 4 * (recon == LQCD_RECON_12 ? 6 : 9) * eb;
     case LQCD_FIELD_SPINOR: return sites * 12 * eb;
     case LQCD_FIELD_CLOVER: return sites * 36 * eb;
+    case LQCD_FIELD_FACE: return (size_t)g.L[0] * g.L[1] * g.L[2] * 6 * eb;
     case LQCD_FIELD_WORKSPACE: {
       size_t sp64 = align256(sites * 12 * sizeof(double2)), sp32 = align256(sites * 12 * sizeof(float2));
       return WS_SPINORS64 * sp64 + WS_SPINORS32 * sp32 + 2 * align256(partial_len(g) * sizeof(double)) + 4096;
@@ -330,10 +338,49 @@ lqcd_status lqcd_clover_build(const lqcd_geom* h, const lqcd_dirac* d, const voi
   REQUIRE(h && d && U64 && clover, "lqcd_clover_build: NULL argument");
   REQUIRE(valid_prec(out_prec) && valid_recon(recon), "lqcd_clover_build: bad precision / recon");
   REQUIRE(clover != U64 && clover_inv != U64 && clover != clover_inv, "lqcd_clover_build: aliased buffers");
+  UNSUPPORTED_ON_SLAB(h, "lqcd_clover_build (use lqcd_clover_build_slab)");
   CloverParm cp;
   cp.kappa = d->kappa; cp.csw = d->csw; cp.ct = d->ct;
   for (int i = 0; i < 3; i++) cp.phiT[i] = h->desc.phiT[i];
   CUDA_TRY(clover_build(h->g, cp, U64, (int)recon, clover, clover_inv, (int)out_prec, as_stream(stream)), "clover_build");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_clover_build_slab(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, lqcd_recon recon,
+                                   const void* halo_lo, const void* halo_hi, void* clover, void* clover_inv,
+                                   lqcd_prec out_prec, void* stream) {
+  REQUIRE(h && d && U64 && clover && halo_lo && halo_hi, "lqcd_clover_build_slab: NULL argument");
+  REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_clover_build_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
+  REQUIRE(valid_prec(out_prec) && valid_recon(recon), "lqcd_clover_build_slab: bad precision / recon");
+  REQUIRE(clover != U64 && clover_inv != U64 && clover != clover_inv, "lqcd_clover_build_slab: aliased buffers");
+  CloverParm cp;
+  cp.kappa = d->kappa; cp.csw = d->csw; cp.ct = 1.0;
+  for (int i = 0; i < 3; i++) cp.phiT[i] = 0.0;
+  CUDA_TRY(clover_build(h->g, cp, U64, (int)recon, clover, clover_inv, (int)out_prec, as_stream(stream), halo_lo, halo_hi),
+           "clover_build (slab)");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_dw_slab_pack(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* in, void* send_lo,
+                              void* send_hi, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && U && in && send_lo && send_hi, "lqcd_dw_slab_pack: NULL argument");
+  REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_dw_slab_pack: the geometry is not a slab (bc != LQCD_BC_SLAB)");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_slab_pack: bad precision / recon");
+  REQUIRE(send_lo != send_hi, "lqcd_dw_slab_pack: aliased face buffers");
+  CUDA_TRY(DISPATCH_PREC(prec, slab_pack<double>(h, dagger != 0, U, (int)recon, in, send_lo, send_hi, as_stream(stream)),
+                         slab_pack<float>(h, dagger != 0, U, (int)recon, in, send_lo, send_hi, as_stream(stream))),
+           "slab_pack kernel");
+  return LQCD_OK;
+}
+
+lqcd_status lqcd_dw_slab_faces(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* recv_lo,
+                               const void* recv_hi, void* out, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && U && recv_lo && recv_hi && out, "lqcd_dw_slab_faces: NULL argument");
+  REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_dw_slab_faces: the geometry is not a slab (bc != LQCD_BC_SLAB)");
+  REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_slab_faces: bad precision / recon");
+  CUDA_TRY(DISPATCH_PREC(prec, slab_faces<double>(h, d->kappa, dagger != 0, U, (int)recon, recv_lo, recv_hi, out, as_stream(stream)),
+                         slab_faces<float>(h, d->kappa, dagger != 0, U, (int)recon, recv_lo, recv_hi, out, as_stream(stream))),
+           "slab_faces kernel");
   return LQCD_OK;
 }
 
@@ -402,6 +449,7 @@ lqcd_status lqcd_dw_eo_apply(const lqcd_geom* h, const lqcd_dirac* d, const void
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_eo_apply: bad precision / recon");
   REQUIRE(out_e != in_e && tmp != in_e && tmp != out_e, "lqcd_dw_eo_apply: aliased buffers");
   REQUIRE(d->mu == 0.0, "lqcd_dw_eo_apply: the even-odd operator does not support a twisted mass (mu != 0)");
+  UNSUPPORTED_ON_SLAB(h, "lqcd_dw_eo_apply");
   CUDA_TRY(DISPATCH_PREC(prec, dw_eo_t<double>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream)),
                          dw_eo_t<float>(h, d, U, clover, clover_inv, in_e, out_e, tmp, dagger != 0, (int)recon, as_stream(stream))),
            "dw_eo kernel");
@@ -559,6 +607,7 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
   REQUIRE(valid_recon(recon), "lqcd_cg_solve: bad recon");
   REQUIRE(f->U64, "lqcd_cg_solve: U64 is required");
   REQUIRE(x != b, "lqcd_cg_solve: x aliases b");
+  UNSUPPORTED_ON_SLAB(h, "lqcd_cg_solve");
   REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve: bad tol / maxiter");
   if (parm->eo) REQUIRE(f->clover64 && f->clover_inv64, "lqcd_cg_solve: eo needs clover64 and clover_inv64");
   if (parm->eo) REQUIRE(d->mu == 0.0, "lqcd_cg_solve: the even-odd solver does not support a twisted mass (mu != 0)");
@@ -671,6 +720,7 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
                                void* out_canon_host, int dagger, lqcd_prec prec, lqcd_recon recon) {
   REQUIRE(desc && d && U_canon_host && in_canon_host && out_canon_host, "lqcd_dw_apply_host: NULL argument");
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply_host: bad precision / recon");
+  REQUIRE(desc->bc != LQCD_BC_SLAB, "lqcd_dw_apply_host: a slab needs its neighbours' faces (lqcd_dw_slab_pack / _faces)");
   lqcd_geom* h = nullptr;
   lqcd_status st = lqcd_geom_create(desc, &h);
   if (st != LQCD_OK) return st;

@@ -48,6 +48,9 @@ struct CloverCtx {
   Geom g;
   const double2* U;
   double phiT[3];
+  // LQCD_BC_SLAB (NEXT-3): the time slices just below and just above the slab, canonical layout [n][4][3][3]
+  const double2* halo_lo;
+  const double2* halo_hi;
 };
 
 // The site a thread works on: tile, local coordinates, parity, global time coordinate.
@@ -98,10 +101,19 @@ __device__ __forceinline__ m3 link_at(const CloverCtx& c, const SitePos& sp, int
     }
   }
   const int p = (sp.par + dm + dn) & 1;
-  const double2* up = c.U + field_offset(g, 4 * NCU, p, t, dir * NCU, local_index(g, l));
   m3 u;
+  if (g.bc == LQCD_BC_SLAB && (x3 < 0 || x3 >= g.L[3])) {   // neighbour rank's slice: from the gauge halo
+    int Tc[4];
+    tile_coords(g, t, Tc);
+    const int n = (Tc[0] * g.b[0] + l[0]) + g.L[0] * ((Tc[1] * g.b[1] + l[1]) + g.L[1] * (Tc[2] * g.b[2] + l[2]));
+    const double2* hp = (x3 < 0 ? c.halo_lo : c.halo_hi) + ((size_t)n * 4 + dir) * 9;
 #pragma unroll
-  for (int k = 0; k < NCU; k++) u.e[k / 3][k % 3] = __ldg(up + (size_t)k * g.TV);
+    for (int k = 0; k < 9; k++) u.e[k / 3][k % 3] = __ldg(hp + k);
+  } else {
+    const double2* up = c.U + field_offset(g, 4 * NCU, p, t, dir * NCU, local_index(g, l));
+#pragma unroll
+    for (int k = 0; k < NCU; k++) u.e[k / 3][k % 3] = __ldg(up + (size_t)k * g.TV);
+  }
   if (RECON == 12) {
 #pragma unroll
     for (int k = 0; k < 3; k++) {
@@ -301,10 +313,12 @@ static cudaError_t clover_launch(const CloverCtx& c, const CloverParm& cp, void*
 }
 
 cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, int recon, void* clover, void* clover_inv,
-                         int out_prec, cudaStream_t s) {
+                         int out_prec, cudaStream_t s, const void* halo_lo, const void* halo_hi) {
   CloverCtx c;
   c.g = g;
   c.U = (const double2*)U64;
+  c.halo_lo = (const double2*)halo_lo;
+  c.halo_hi = (const double2*)halo_hi;
   for (int i = 0; i < 3; i++) c.phiT[i] = cp.phiT[i];
   const bool f64 = out_prec == LQCD_F64, r12 = recon == 12, inv = clover_inv != nullptr;
 #define LQCD_CLV(T, R, I) return clover_launch<T, R, I>(c, cp, clover, clover_inv, s)

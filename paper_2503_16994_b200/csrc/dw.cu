@@ -236,15 +236,13 @@ __device__ __forceinline__ void dw_body(const Geom& g, const DwArgs<T>& a) {
           bool cr = (l[3] + 1 == g.b[3]);
           int jn = cr ? j - (g.b[3] - 1) * st3 : j + st3;
           int tn = cr ? __ldg(tab + 6) : tile;
-          int xn = (x3 + 1 == g.L[3]) ? 0 : x3 + 1;
-          if (!(nonper && frozen_slice(g, xn)))
+          if (!(nonper && time_hop_blocked(g, x3, true)))
             hop_dir<T, RECON, 3, true>(a.in + field_offset(g, 12, q, tn, 0, jn),
                                        a.U + ubase_self + (size_t)(3 * NCU) * TV, TV, TV, sg, a.has_theta, a.theta[3], acc);
           cr = (l[3] == 0);
           jn = cr ? j + (g.b[3] - 1) * st3 : j - st3;
           tn = cr ? __ldg(tab + 7) : tile;
-          xn = (x3 == 0) ? g.L[3] - 1 : x3 - 1;
-          if (!(nonper && frozen_slice(g, xn)))
+          if (!(nonper && time_hop_blocked(g, x3, false)))
             hop_dir<T, RECON, 3, false>(a.in + field_offset(g, 12, q, tn, 0, jn),
                                         a.U + field_offset(g, 4 * NCU, q, tn, 3 * NCU, jn), TV, TV, -sg, a.has_theta,
                                         a.theta[3], acc);
@@ -456,7 +454,7 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
     if (MU == 0) jn = j - l0h + ((l[0] + 1) >> 1);
     else jn = j + stride;
     bool on = true;
-    if (MU == 3 && nonper) on = !frozen_slice(g, (x3 + 1 == g.L[3]) ? 0 : x3 + 1);
+    if (MU == 3 && nonper) on = !time_hop_blocked(g, x3, true);
     if (on) {
       const T2<T>* ps = cr ? hb + fq : sp + (q * 12) * TV + jn;
       hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, TV, TV, sg, a.has_theta, a.theta[MU], acc);
@@ -469,7 +467,7 @@ __device__ __forceinline__ void hop_pair(const Geom& g, const DwArgs<T>& a, cons
     if (MU == 0) jn = j - l0h + ((l[0] - 1) >> 1);
     else jn = j - stride;
     bool on = true;
-    if (MU == 3 && nonper) on = !frozen_slice(g, (x3 == 0) ? g.L[3] - 1 : x3 - 1);
+    if (MU == 3 && nonper) on = !time_hop_blocked(g, x3, false);
     if (on) {
       const T2<T>* ps = cr ? hb + 12 * TV + fq : sp + (q * 12) * TV + jn;
       const T2<T>* us = cr ? hb + 24 * TV + fq : ub + (q * NCU) * TV + jn;

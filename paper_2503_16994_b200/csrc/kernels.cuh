@@ -18,8 +18,18 @@ struct CloverParm {
   double kappa, csw, ct;
   double phiT[3];
 };
+// halo_lo / halo_hi: LQCD_BC_SLAB only (the neighbour ranks' adjacent time slices, canonical fp64 layout)
 cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, int recon, void* clover, void* clover_inv,
-                         int out_prec, cudaStream_t s);
+                         int out_prec, cudaStream_t s, const void* halo_lo = nullptr, const void* halo_hi = nullptr);
+
+// slab.cu (NEXT-3): half-spinor faces of a time slab; [6][L1 L2 L3] complex numbers each
+}  // namespace lqcd
+struct lqcd_geom;
+namespace lqcd {
+template <typename T> cudaError_t slab_pack(const lqcd_geom* h, bool dagger, const void* U, int recon, const void* in,
+                                            void* send_lo, void* send_hi, cudaStream_t s);
+template <typename T> cudaError_t slab_faces(const lqcd_geom* h, double kappa, bool dagger, const void* U, int recon,
+                                             const void* recv_lo, const void* recv_hi, void* out, cudaStream_t s);
 
 // blas.cu -- CG scalars live on the device
 struct CgState {

@@ -86,6 +86,15 @@ __host__ __device__ inline bool frozen_slice(const Geom& g, int x3) {
   return false;
 }
 
+// Is the time hop out of slice x3 (fwd: to x3 + 1, else to x3 - 1, wrapping) NOT taken by the stencil kernels?
+// open / SF: hops onto frozen slices (D7).  Slab: hops across the slab's two time
+// faces -- the face kernels of slab.cu add them from the exchanged half spinors.
+__host__ __device__ inline bool time_hop_blocked(const Geom& g, int x3, bool fwd) {
+  if (g.bc == LQCD_BC_SLAB) return fwd ? (x3 + 1 == g.L[3]) : (x3 == 0);
+  const int xn = fwd ? ((x3 + 1 == g.L[3]) ? 0 : x3 + 1) : ((x3 == 0) ? g.L[3] - 1 : x3 - 1);
+  return frozen_slice(g, xn);
+}
+
 // element offset (in complex numbers) of component c, site j of tile `tile`, parity p, NC comps/site
 __host__ __device__ inline size_t field_offset(const Geom& g, int NC, int p, int tile, int c, int j) {
   return ((size_t)p * g.Vh + (size_t)tile * g.TV) * NC + (size_t)c * g.TV + j;

@@ -1,0 +1,152 @@
+"""-m gpu parity of the time-direction domain decomposition: the lattice is cut into
+P time slabs, each with its own LQCD_BC_SLAB geometry, fields, clover term (built from the slab plus a one-slice
+gauge halo) and face buffers, exactly as P ranks would hold them; the slabs run one after the other on the one GPU
+(no kernel waits on another), the faces are moved between them by plain copies in the pattern slab.FaceExchange uses
+between ranks (tests/test_slab_dist.py checks that pattern over gloo).  The assembled result must be the oracle's D
+(D^+) on the whole lattice, to north_star's per-site tolerances."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2503_16994_b200 import binding as B
+from paper_2503_16994_b200 import slab, synth
+
+from gpu_util import round_f32, site_rel_err, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL = {B.F64: 1e-12, B.F32: 2e-6}
+
+
+@pytest.fixture
+def mode(request):
+    B.set_option("dw_mode", request.param)
+    yield request.param
+    B.set_option("dw_mode", "pipe")
+
+
+class Rank:
+    """What one rank of the decomposition holds."""
+
+    def __init__(self, L, P, r, theta, U, kappa, csw, prec, recon):
+        self.T = slab.slab_extent(L[3], P)
+        self.ns = L[0] * L[1] * L[2]
+        self.lo, self.hi = r * self.T * self.ns, (r + 1) * self.T * self.ns   # canonical site range (time slowest)
+        self.g = slab.slab_geom_create(L, P, theta)
+        Uc = to_dev(U[self.lo:self.hi])
+        self.U64 = B.alloc_field(self.g, B.FIELD_GAUGE, B.F64, recon)
+        B.gauge_import(self.g, Uc, self.U64, B.F64, recon)
+        self.U = self.U64
+        if prec == B.F32:
+            self.U = B.alloc_field(self.g, B.FIELD_GAUGE, prec, recon)
+            B.gauge_import(self.g, Uc, self.U, prec, recon)
+        V = U.shape[0]
+        below = np.arange(self.lo - self.ns, self.lo) % V
+        above = np.arange(self.hi, self.hi + self.ns) % V
+        self.A = B.alloc_field(self.g, B.FIELD_CLOVER, prec)
+        B.clover_build_slab(self.g, kappa, csw, self.U64, to_dev(U[below]), to_dev(U[above]), self.A, None, recon, prec)
+        self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (B.alloc_field(self.g, B.FIELD_FACE, prec) for _ in range(4))
+        self.src = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
+        self.dst = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
+
+
+def slab_dw(ranks, kappa, psi, prec, recon, dagger, clover=True, mu=0.0):
+    P = len(ranks)
+    for R in ranks:
+        B.spinor_import(R.g, to_dev(psi[R.lo:R.hi]), R.src, prec)
+        R.dst.fill_(0x7F)
+        B.dw_slab_pack(R.g, kappa, R.U, R.src, R.send_lo, R.send_hi, dagger, prec, recon)
+    for r, R in enumerate(ranks):   # the ring: send_lo -> below's recv_hi, send_hi -> above's recv_lo
+        ranks[(r - 1) % P].recv_hi.copy_(R.send_lo)
+        ranks[(r + 1) % P].recv_lo.copy_(R.send_hi)
+    out = np.empty_like(psi)
+    for R in ranks:
+        fn = B.dwdag_apply if dagger else B.dw_apply
+        fn(R.g, kappa, R.U, R.A if clover else None, R.src, R.dst, prec, recon, mu=mu)
+        B.dw_slab_faces(R.g, kappa, R.U, R.recv_lo, R.recv_hi, R.dst, dagger, prec, recon)
+        o = torch.empty((R.hi - R.lo, 4, 3), dtype=torch.complex128, device="cuda")
+        B.spinor_export(R.g, R.dst, o, prec)
+        torch.cuda.synchronize()
+        out[R.lo:R.hi] = o.cpu().numpy()
+    return out
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream", "split", "direct"], indirect=True)
+@pytest.mark.parametrize("L,P,theta", [
+    ((8, 4, 4, 8), 2, (0.3, -0.2, 0.1, np.pi)),     # two slabs of 4^4 tiles, antiperiodic in time
+    ((4, 8, 4, 12), 3, None),                        # three slabs
+    ((6, 4, 10, 8), 1, (0.5, 0.5, 0.5, 1.0)),        # one slab = the periodic lattice through its own faces; no 4^4 tiles
+    ((4, 4, 4, 16), 2, (0, 0, 0, np.pi)),            # slabs of two tiles in time
+])
+@pytest.mark.parametrize("prec,recon", [(B.F64, B.RECON_18), (B.F64, B.RECON_12), (B.F32, B.RECON_18)])
+def test_slab_dw_equals_whole_lattice(mode, L, P, theta, prec, recon):
+    kappa, csw = 0.137, 1.9
+    U = synth.smooth_gauge(L, 101)
+    psi = synth.gaussian_spinor(L, 102)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    Uo, psio, Ao = (round_f32(U), round_f32(psi), round_f32(A)) if prec == B.F32 else (U, psi, A)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, prec, recon) for r in range(P)]
+    # the clover term of each slab is the whole lattice's (fp64 build, rounded once)
+    for R in ranks:
+        got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
+        B.clover_export(R.g, R.A, got, prec)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+    for dagger in (False, True):
+        ref = oracle.dw(L, Uo, psio, kappa, Ao, theta=theta, dagger=dagger)
+        assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, dagger), ref) <= TOL[prec]
+    ref = oracle.dw(L, Uo, psio, kappa, None, theta=theta)
+    assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, False, clover=False), ref) <= TOL[prec]
+    ref = oracle.dw(L, Uo, psio, kappa, Ao, theta=theta, dagger=True, mu=0.3)
+    assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, True, mu=0.3), ref) <= TOL[prec]
+    for R in ranks:
+        B.geom_destroy(R.g)
+
+
+def test_slab_without_faces_differs_and_unsupported_calls_fail():
+    """The slab stencil alone must NOT be the periodic operator (the faces are really needed), and the calls that
+    would ignore the faces are refused."""
+    L, kappa = (4, 4, 4, 8), 0.13
+    U = synth.smooth_gauge(L, 103)
+    psi = synth.gaussian_spinor(L, 104)
+    R = Rank(L, 1, 0, None, U, kappa, 1.0, B.F64, B.RECON_18)
+    B.spinor_import(R.g, to_dev(psi), R.src, B.F64)
+    B.dw_apply(R.g, kappa, R.U, R.A, R.src, R.dst)
+    o = torch.empty((psi.shape[0], 4, 3), dtype=torch.complex128, device="cuda")
+    B.spinor_export(R.g, R.dst, o, B.F64)
+    torch.cuda.synchronize()
+    ref = oracle.dw(L, U, psi, kappa, oracle.clover_blocks(L, U, kappa, 1.0))
+    err = np.linalg.norm((o.cpu().numpy() - ref).reshape(psi.shape[0], -1), axis=1)
+    t = np.arange(psi.shape[0]) // (4 * 4 * 4)
+    assert np.all(err[(t > 0) & (t < 7)] < 1e-12) and np.all(err[(t == 0) | (t == 7)] > 1e-3)
+    ws = B.alloc_field(R.g, B.FIELD_WORKSPACE)
+    for call in (lambda: B.cg_solve(R.g, kappa, R.U, R.A, R.src, R.dst, ws),
+                 lambda: B.clover_build(R.g, kappa, 1.0, R.U, R.A),
+                 lambda: B.dw_eo_apply(R.g, kappa, R.U, R.A, R.A, R.src, R.dst, ws)):
+        with pytest.raises(B.LqcdError) as e:
+            call()
+        assert e.value.status == B.EUNSUPPORTED
+    per = B.geom_create(L)
+    with pytest.raises(B.LqcdError):   # the face kernels want a slab geometry
+        B.dw_slab_pack(per, kappa, R.U, R.src, R.send_lo, R.send_hi)
+    B.geom_destroy(per)
+    B.geom_destroy(R.g)
+
+
+def test_slab_dirac_driver_single_rank():
+    """slab.SlabDirac (pack -> exchange on a side stream || stencil -> faces) with one rank: the periodic lattice."""
+    L, kappa, csw, theta = (8, 8, 4, 8), 0.135, 1.7, (0, 0, 0, np.pi)
+    U = synth.smooth_gauge(L, 105)
+    psi = synth.gaussian_spinor(L, 106)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    R = Rank(L, 1, 0, theta, U, kappa, csw, B.F64, B.RECON_18)
+    D = slab.SlabDirac(R.g, kappa, R.U, R.A)
+    B.spinor_import(R.g, to_dev(psi), R.src, B.F64)
+    for dagger in (False, True):
+        D.apply(R.src, R.dst, dagger)
+        o = torch.empty((psi.shape[0], 4, 3), dtype=torch.complex128, device="cuda")
+        B.spinor_export(R.g, R.dst, o, B.F64)
+        torch.cuda.synchronize()
+        assert site_rel_err(o.cpu().numpy(), oracle.dw(L, U, psi, kappa, A, theta=theta, dagger=dagger)) <= 1e-12
+    B.geom_destroy(R.g)
