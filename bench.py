@@ -164,6 +164,7 @@ class Setup:
         self.V = synth.vol(L)
         dev = torch.device("cuda", torch.cuda.current_device())
         self.g = B.geom_create(L, bc, theta, synth.SF_PHI0 if sf else None, phiT, device=dev.index)
+        self.theta_is_zero = bc == B.BC_PERIODIC and (theta is None or not any(theta))
         Uc = synth.smooth_gauge_torch(L, synth.seed_for(seed_cfg, 0) + 100 * rank, dev)
         if sf:
             n0 = L[0] * L[1] * L[2]
@@ -402,6 +403,21 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
     rows["next2_correlator_ps_12cols_f64"] = {"ms": round(ms, 3), "GB/s": gbs(24 * nrhs, 8, ms),
                                               "frac_measured_peak": round(gbs(24 * nrhs, 8, ms) / peak, 4)}
     del src, dst, wsc
+    # NEXT-3: the same lattice as ONE time slab -- pack, face exchange with itself (the periodic
+    # wrap) on a side stream, stencil without the two face hops, face kernel.  What a rank of a decomposed lattice
+    # runs per application; the difference to a4 is the whole cost of the decomposition on the GPU side.
+    if S.theta_is_zero:
+        from paper_2503_16994_b200 import slab
+        gs = slab.slab_geom_create(L, 1, None, device=torch.cuda.current_device())
+        D = slab.SlabDirac(gs, kappa, S.U[(B.F64, recon)], S.A[B.F64], B.F64, recon)
+        ms = time_calls(torch, lambda: D.apply(S.psi[B.F64], S.out[B.F64]), 10)
+        ms0 = dw["dw_f64_recon%d" % recon]["ms"]
+        rows["next3_slab_dw_f64_world1"] = {
+            "ms": round(ms, 4), "GFLOP/s": round(FLOP_DW * V / ms / 1e6, 1), "GB/s": gbs(REALS_DW[recon], 8, ms),
+            "overhead_vs_a4": round(ms / ms0 - 1.0, 4), "face_bytes_per_application": 2 * B.field_bytes(gs, B.FIELD_FACE, B.F64),
+            "note": "lqcd_dw_slab_pack + self-exchange + lqcd_dw_apply (BC_SLAB) + lqcd_dw_slab_faces"}
+        del D
+        B.geom_destroy(gs)
     # a6: BLAS-1 reduction alone (|v|^2 over one spinor)
     ws = B.alloc_field(g, B.FIELD_WORKSPACE)
     ms = time_calls(torch, lambda: B.spinor_norm2(g, S.psi[B.F64], ws), 10)
@@ -418,6 +434,21 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
                                    "GB/s_model": gbs(REALS_CG_ITER[recon], 8, ms_it),
                                    "frac_measured_peak": round(gbs(REALS_CG_ITER[recon], 8, ms_it) / peak, 4),
                                    "model": "%d reals/site/iteration (fused plan, SURVEY.md 8(d))" % REALS_CG_ITER[recon]}
+    if S.theta_is_zero:   # NEXT-3: the slab solver's iteration (unfused BLAS-1, two all-reduces) on one slab
+        from paper_2503_16994_b200 import slab
+        gs = slab.slab_geom_create(L, 1, None, device=torch.cuda.current_device())
+        comm = slab.SlabCommunicator(gs)
+        for n in (10, 40):
+            info = slab.cg_solve_slab(gs, kappa, S.U[(B.F64, recon)], S.A[B.F64], b, x, ws, comm, tol=1e-30, maxiter=n,
+                                      check_every=n, recon=recon, raise_on_notconv=False)
+            t[n] = info["seconds"]
+        ms_sl = (t[40] - t[10]) / 30 * 1e3
+        rows["next3_slab_cg_iteration_f64_world1"] = {
+            "ms_per_iteration": round(ms_sl, 4), "vs_a7": round(ms_sl / ms_it, 4),
+            "note": "lqcd_cg_solve_slab: pack / exchange / stencil / faces per operator, r -= alpha q and |r|^2 in a "
+                    "separate pass, scalars through the all-reduce callback"}
+        del comm
+        B.geom_destroy(gs)
     del ws
     torch.cuda.empty_cache()
     rows.update(run_config2(torch, B, synth, peak))

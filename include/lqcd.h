@@ -180,6 +180,31 @@ lqcd_status lqcd_clover_build_slab(const lqcd_geom* g, const lqcd_dirac* d, cons
                                    const void* halo_lo, const void* halo_hi, void* clover, void* clover_inv,
                                    lqcd_prec out_prec, void* stream);
 
+/* CG! on the slabs of a decomposed lattice (8(e)(ii): "CG adds two scalar all-reduces per iteration"): the algorithm
+ * of lqcd_cg_solve (plain fp64, not even-odd) with D applied as pack / exchange / stencil / faces and every inner
+ * product summed over the ranks.  All ranks call it together with their slab's fields.  The library does no
+ * communication itself: the caller supplies three host callbacks, each called while the library enqueues work on
+ * `stream`, each returning 0 on success (nonzero aborts the solve with LQCD_ECUDA on that rank):
+ *   exchange_start(ctx): send_lo / send_hi have been written by work already enqueued on `stream`; start moving send_lo
+ *                        into the rank below's recv_hi and send_hi into the rank above's recv_lo (ordered after
+ *                        `stream`'s current tail, e.g. on a second stream so that it overlaps the stencil kernel);
+ *   exchange_wait(ctx) : make `stream` wait until recv_lo / recv_hi have arrived;
+ *   allreduce_sum(ctx, n): sum scalars[0..n) (DEVICE doubles, written by work enqueued on `stream`) over all ranks,
+ *                        in place, ordered on `stream`.
+ * Face buffers and scalars (>= 4 doubles): DEVICE, caller-owned.  b, x: this rank's slab of the source / solution.
+ * info as lqcd_cg_solve (the residuals are those of the whole lattice).  parm->mixed and parm->eo must be 0. */
+typedef struct {
+  void* send_lo; void* send_hi; void* recv_lo; void* recv_hi;
+  double* scalars;
+  int (*exchange_start)(void* ctx);
+  int (*exchange_wait)(void* ctx);
+  int (*allreduce_sum)(void* ctx, int n);
+  void* ctx;
+} lqcd_slab_comm;
+lqcd_status lqcd_cg_solve_slab(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, const void* clover64,
+                               const void* b, void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
+                               const lqcd_slab_comm* comm, lqcd_recon recon, void* stream);
+
 /* SURVEY.md 8(f) NEXT-1 (the 12 colour-spin sources of propagator! share one gauge field): D or D^+
  * (dagger != 0) applied to nrhs (1..64) spinor fields in one pass.  in / out: DEVICE arrays of nrhs internal spinor
  * fields stored back to back (lqcd_field_bytes(SPINOR) apart), caller-owned, not overlapping.  Links and clover

@@ -24,7 +24,7 @@ EXPORTS = [
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
     "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
-    "lqcd_clover_build_slab",
+    "lqcd_clover_build_slab", "lqcd_cg_solve_slab",
 ]
 
 
@@ -241,6 +241,30 @@ def cg_solve(g, kappa, U64, clover64, b, x, workspace, tol=1e-10, maxiter=10000,
     info = CgInfo()
     st = lib().lqcd_cg_solve(g, ctypes.byref(d), ctypes.byref(f), _ptr(b), _ptr(x), _ptr(workspace), ctypes.byref(p),
                              ctypes.byref(info), recon, _stream(stream))
+    if st != OK and not (st == ENOTCONV and not raise_on_notconv):
+        _check(st)
+    return _info_dict(info, st)
+
+
+SLAB_CALLBACK = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
+SLAB_CALLBACK_N = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int)
+
+
+class SlabComm(ctypes.Structure):
+    """lqcd_slab_comm: face buffers, the all-reduce payload and the three host callbacks."""
+    _fields_ = [("send_lo", ctypes.c_void_p), ("send_hi", ctypes.c_void_p), ("recv_lo", ctypes.c_void_p),
+                ("recv_hi", ctypes.c_void_p), ("scalars", ctypes.c_void_p), ("exchange_start", SLAB_CALLBACK),
+                ("exchange_wait", SLAB_CALLBACK), ("allreduce_sum", SLAB_CALLBACK_N), ("ctx", ctypes.c_void_p)]
+
+
+def cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, comm, tol=1e-10, maxiter=10000, check_every=16,
+                  recon=RECON_18, stream=None, raise_on_notconv=True, mu=0.0):
+    """lqcd_cg_solve_slab; comm: a SlabComm (paper_2503_16994_b200.slab.make_comm builds one)."""
+    d = _dirac(kappa, mu=mu)
+    p = CgParm(float(tol), int(maxiter), 0, 0, 1e-4, int(check_every))
+    info = CgInfo()
+    st = lib().lqcd_cg_solve_slab(g, ctypes.byref(d), _ptr(U64), _ptr(clover64), _ptr(b), _ptr(x), _ptr(workspace),
+                                  ctypes.byref(p), ctypes.byref(info), ctypes.byref(comm), recon, _stream(stream))
     if st != OK and not (st == ENOTCONV and not raise_on_notconv):
         _check(st)
     return _info_dict(info, st)

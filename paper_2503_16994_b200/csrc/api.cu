@@ -701,6 +701,130 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
   return st;
 }
 
+}  // extern "C"
+
+// ---- NEXT-3: CG over the time slabs of a decomposed lattice -------------------------------------------------------
+namespace {
+struct SlabSolve {
+  const lqcd_geom* h;
+  const lqcd_dirac* d;
+  const void* U;
+  const void* A;
+  int recon;
+  const lqcd_slab_comm* comm;
+  double* partial;
+  cudaStream_t s;
+
+  lqcd_status cb(int rc, const char* what) const {
+    if (rc != 0) { set_error("lqcd_cg_solve_slab: callback %s failed (%d)", what, rc); return LQCD_ECUDA; }
+    return LQCD_OK;
+  }
+  // out = D in (D^+ in) on this rank's slab, faces included
+  lqcd_status apply(const void* in, void* out, bool dagger) const {
+    CKS(slab_pack<double>(h, dagger, U, recon, in, comm->send_lo, comm->send_hi, s), "slab_pack");
+    lqcd_status st = cb(comm->exchange_start(comm->ctx), "exchange_start");
+    if (st != LQCD_OK) return st;
+    Op<double> M;
+    M.geom = h; M.U = U; M.A = A; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.mu = d->mu; M.recon = recon; M.eo = false;
+    CKS(M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "slab stencil");
+    st = cb(comm->exchange_wait(comm->ctx), "exchange_wait");
+    if (st != LQCD_OK) return st;
+    CKS(slab_faces<double>(h, d->kappa, dagger, U, recon, comm->recv_lo, comm->recv_hi, out, s), "slab_faces");
+    return LQCD_OK;
+  }
+  // scalars[0] = sum over ranks of the `nblocks` partial sums in `partial`
+  lqcd_status reduce(int nblocks) const {
+    CKS(final_sum(partial, nblocks, 1, comm->scalars, s), "final_sum");
+    return cb(comm->allreduce_sum(comm->ctx, 1), "allreduce_sum");
+  }
+  lqcd_status norm2(const void* v, size_t n, double* host) const {
+    CKS(norm2_partial<double>(v, n, partial, s), "norm2");
+    lqcd_status st = reduce(reduce_blocks(n));
+    if (st != LQCD_OK) return st;
+    if (host) {
+      CKS(cudaMemcpyAsync(host, comm->scalars, sizeof(double), cudaMemcpyDeviceToHost, s), "copy scalar");
+      CKS(cudaStreamSynchronize(s), "sync");
+    }
+    return LQCD_OK;
+  }
+};
+#define LSS(e) do { lqcd_status _st = (e); if (_st != LQCD_OK) return _st; } while (0)
+}  // namespace
+
+extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, const void* clover64,
+                                          const void* b, void* x, void* workspace, const lqcd_cg_parm* parm,
+                                          lqcd_cg_info* info, const lqcd_slab_comm* comm, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && U64 && b && x && workspace && parm && info && comm, "lqcd_cg_solve_slab: NULL argument");
+  REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_cg_solve_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
+  REQUIRE(valid_recon(recon), "lqcd_cg_solve_slab: bad recon");
+  REQUIRE(x != b, "lqcd_cg_solve_slab: x aliases b");
+  REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve_slab: bad tol / maxiter");
+  REQUIRE(!parm->mixed && !parm->eo, "lqcd_cg_solve_slab: plain fp64 CG only (mixed and eo must be 0)");
+  REQUIRE(comm->send_lo && comm->send_hi && comm->recv_lo && comm->recv_hi && comm->scalars, "lqcd_cg_solve_slab: NULL comm buffer");
+  REQUIRE(comm->exchange_start && comm->exchange_wait && comm->allreduce_sum, "lqcd_cg_solve_slab: NULL callback");
+  memset(info, 0, sizeof(*info));
+  auto t0 = std::chrono::steady_clock::now();
+  const Geom& g = h->g;
+  cudaStream_t s = as_stream(stream);
+  Workspace ws{(char*)workspace, 0};
+  const size_t sites = (size_t)2 * g.Vh;
+  void* v64[WS_SPINORS64];
+  for (int i = 0; i < WS_SPINORS64; i++) v64[i] = ws.take(sites * 12 * sizeof(double2));
+  for (int i = 0; i < WS_SPINORS32; i++) ws.take(sites * 12 * sizeof(float2));
+  double* partial = (double*)ws.take(partial_len(g) * sizeof(double));
+  ws.take(64);
+  CgState* state = (CgState*)ws.take(sizeof(CgState));
+  const size_t n = spinor_complex(g);
+  const size_t bytes = n * sizeof(double2);
+  SlabSolve S{h, d, U64, clover64, (int)recon, comm, partial, s};
+  void *r = v64[0], *p = v64[1], *t = v64[2], *q = v64[3], *bp = v64[4];
+
+  LSS(S.apply(b, bp, true));                                   // b' = D^+ b
+  CKS(cudaMemsetAsync(x, 0, bytes, s), "memset");
+  CKS(cudaMemcpyAsync(r, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+  CKS(cudaMemcpyAsync(p, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+  LSS(S.norm2(r, n, nullptr));
+  CKS(cg_init_state(state, comm->scalars, 1, parm->tol, s), "cg_init_state");
+  const int check = parm->check_every > 0 ? parm->check_every : 16;
+  CgState hs;
+  int launched = 0;
+  for (;;) {   // every rank sees the same all-reduced scalars, hence the same state: the ranks stay in lockstep
+    CKS(cudaMemcpyAsync(&hs, state, sizeof(CgState), cudaMemcpyDeviceToHost, s), "copy state");
+    CKS(cudaStreamSynchronize(s), "sync");
+    if (hs.done || launched >= parm->maxiter) break;
+    int batch = check;
+    if (launched + batch > parm->maxiter) batch = parm->maxiter - launched;
+    for (int it = 0; it < batch; it++) {
+      LSS(S.apply(p, t, false));
+      CKS(norm2_partial<double>(t, n, partial, s), "norm2");
+      LSS(S.reduce(reduce_blocks(n)));
+      CKS(cg_reduce_alpha(state, comm->scalars, 1, s), "alpha");
+      LSS(S.apply(t, q, true));
+      CKS(cg_raxpy_norm<double>(state, q, r, n, partial, s), "r -= alpha q");
+      LSS(S.reduce(reduce_blocks(n)));
+      CKS(cg_reduce_beta(state, comm->scalars, 1, s), "beta");
+      CKS(cg_update_xp<double>(state, x, p, r, n, s), "update");
+    }
+    launched += batch;
+  }
+  info->iters = hs.iters;
+  if (hs.breakdown) { set_error("lqcd_cg_solve_slab: breakdown (NaN or <p,D^+D p> <= 0) at iteration %d", hs.iters); return LQCD_EBREAKDOWN; }
+  // true residuals with fresh operator applications (R11), norms over the whole lattice
+  double nb = 0, nr = 0, nq = 0;
+  LSS(S.apply(x, t, false));
+  CKS(xmy<double>(b, t, t, n, s), "b - Dx");
+  LSS(S.norm2(b, n, &nb));
+  LSS(S.norm2(t, n, &nr));
+  LSS(S.apply(t, q, true));
+  LSS(S.norm2(q, n, &nq));
+  info->rel_resid_true = nb > 0 ? sqrt(nr / nb) : 0.0;
+  info->rel_resid_normal = hs.rho0 > 0 ? sqrt(nq / hs.rho0) : 0.0;
+  info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  if (!hs.done) { set_error("lqcd_cg_solve_slab: not converged after %d iterations", hs.iters); return LQCD_ENOTCONV; }
+  return LQCD_OK;
+}
+
+extern "C" {
 lqcd_status lqcd_propagator(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4], void* columns,
                             void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info infos[12], lqcd_recon recon, void* stream) {
   REQUIRE(h && d && f && y && columns && workspace && parm && infos, "lqcd_propagator: NULL argument");

@@ -130,6 +130,25 @@ __global__ void cg_update_xp_kernel(const CgState* st, T2<T>* x, T2<T>* p, const
   }
 }
 
+// r -= alpha q with alpha on the device, |r|^2 partial per CTA (the unfused form of EPI_AXPY_NORM, used by the slab
+// solver, whose operator result is complete only after the face kernel); does nothing once st->done is set
+template <typename T>
+__global__ void cg_raxpy_norm_kernel(const CgState* st, const T2<T>* __restrict__ q, T2<T>* r, size_t n, double* partial) {
+  __shared__ double s_red[32];
+  if (st->done) return;
+  const T al = (T)st->alpha;
+  double acc = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> qv = q[i], rv = r[i];
+    rv.x = fma(-al, qv.x, rv.x);
+    rv.y = fma(-al, qv.y, rv.y);
+    r[i] = rv;
+    acc += (double)rv.x * (double)rv.x + (double)rv.y * (double)rv.y;
+  }
+  double s = block_sum(acc, s_red);
+  if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
 template <typename T>
 __global__ void axpy_kernel(T a, const T2<T>* __restrict__ x, T2<T>* y, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -214,6 +233,11 @@ template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void*
   count_launch();
   return cudaGetLastError();
 }
+template <typename T> cudaError_t cg_raxpy_norm(const CgState* st, const void* q, void* r, size_t n, double* partial, cudaStream_t s) {
+  cg_raxpy_norm_kernel<T><<<reduce_blocks(n), RB_THREADS, 0, s>>>(st, (const T2<T>*)q, (T2<T>*)r, n, partial);
+  count_launch();
+  return cudaGetLastError();
+}
 template <typename T> cudaError_t axpy(double a, const void* x, void* y, size_t n, cudaStream_t s) {
   axpy_kernel<T><<<ew_blocks(n), 256, 0, s>>>((T)a, (const T2<T>*)x, (T2<T>*)y, n);
   count_launch();
@@ -241,6 +265,7 @@ template <typename T> cudaError_t mask_frozen(const Geom& g, void* psi, cudaStre
   template cudaError_t dot_partial<T>(const void*, const void*, size_t, double*, cudaStream_t);     \
   template cudaError_t cg_update_xp<T>(const CgState*, void*, void*, const void*, size_t, cudaStream_t); \
   template cudaError_t axpy<T>(double, const void*, void*, size_t, cudaStream_t);                   \
+  template cudaError_t cg_raxpy_norm<T>(const CgState*, const void*, void*, size_t, double*, cudaStream_t); \
   template cudaError_t xmy<T>(const void*, const void*, void*, size_t, cudaStream_t);               \
   template cudaError_t mask_frozen<T>(const Geom&, void*, cudaStream_t);
 INST(double)

@@ -49,6 +49,8 @@ cudaError_t cg_reduce_alpha(CgState* st, const double* partial, int n, cudaStrea
 cudaError_t cg_reduce_beta(CgState* st, const double* partial, int n, cudaStream_t s);
 // x += alpha p ; p = r + beta p   (skips according to st->done)
 template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void* p, const void* r, size_t ncomplex, cudaStream_t s);
+// r -= st->alpha * q, |r|^2 partials (reduce_blocks(ncomplex) of them); skipped once st->done is set
+template <typename T> cudaError_t cg_raxpy_norm(const CgState* st, const void* q, void* r, size_t ncomplex, double* partial, cudaStream_t s);
 // y = a*x + y  /  y = x + a*y  / copy / zero with host scalar a
 template <typename T> cudaError_t axpy(double a, const void* x, void* y, size_t ncomplex, cudaStream_t s);
 template <typename T> cudaError_t xmy(const void* x, const void* y, void* z, size_t ncomplex, cudaStream_t s);  // z = x - y

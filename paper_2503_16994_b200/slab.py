@@ -130,3 +130,54 @@ def gauge_halo_exchange(U_canon_slab, L, exchange=None):
     # my first slice is the halo_hi of the rank below; my last slice the halo_lo of the rank above
     xch(first, last, halo_lo, halo_hi)
     return halo_lo, halo_hi
+
+
+class SlabCommunicator:
+    """One rank's lqcd_slab_comm: fp64 face buffers, the all-reduce payload and the three host callbacks that
+    lqcd_cg_solve_slab calls.  Call the solver with stream=None (torch's current stream): the callbacks order their
+    work against that stream.  The face exchange runs on a stream of its own and overlaps the interior stencil."""
+
+    def __init__(self, g, exchange=None):
+        import ctypes
+        import sys
+        import traceback
+
+        import torch
+
+        xch = exchange if exchange is not None else FaceExchange()
+        self.exchange = xch
+        self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (B.alloc_field(g, B.FIELD_FACE, B.F64) for _ in range(4))
+        self.scalars = torch.zeros(4, dtype=torch.float64, device=self.send_lo.device)
+        self.comm_stream = torch.cuda.Stream()
+
+        def guarded(fn):
+            def wrapper(*a):
+                try:
+                    fn(*a)
+                    return 0
+                except Exception:   # an exception must not unwind through the C frames
+                    traceback.print_exc(file=sys.stderr)
+                    return 1
+            return wrapper
+
+        def start(_ctx):
+            self.comm_stream.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(self.comm_stream):
+                xch.finish(xch.start(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi))
+
+        def wait(_ctx):
+            torch.cuda.current_stream().wait_stream(self.comm_stream)
+
+        def allreduce(_ctx, n):
+            xch.allreduce_sum(self.scalars[:n])
+
+        # keep the CFUNCTYPE objects alive as long as the struct
+        self._cbs = (B.SLAB_CALLBACK(guarded(start)), B.SLAB_CALLBACK(guarded(wait)), B.SLAB_CALLBACK_N(guarded(allreduce)))
+        self.struct = B.SlabComm(self.send_lo.data_ptr(), self.send_hi.data_ptr(), self.recv_lo.data_ptr(),
+                                 self.recv_hi.data_ptr(), self.scalars.data_ptr(), self._cbs[0], self._cbs[1],
+                                 self._cbs[2], ctypes.c_void_p(None))
+
+
+def cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, communicator, **kw):
+    """D x = b on the decomposed lattice; every rank calls this with its slab.  Returns lqcd_cg_solve's info dict."""
+    return B.cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, communicator.struct, **kw)

@@ -150,3 +150,106 @@ def test_slab_dirac_driver_single_rank():
         torch.cuda.synchronize()
         assert site_rel_err(o.cpu().numpy(), oracle.dw(L, U, psi, kappa, A, theta=theta, dagger=dagger)) <= 1e-12
     B.geom_destroy(R.g)
+
+
+class ThreadRing:
+    """Test stand-in for slab.FaceExchange between P 'ranks' that are threads of this process sharing the one GPU and
+    its default stream: host barriers order the enqueues, stream order and events order the work, so no kernel ever
+    spins on another.
+    Same interface and the same who-gets-what as FaceExchange."""
+
+    def __init__(self, P):
+        import threading
+        self.P = P
+        self.barrier = threading.Barrier(P, timeout=120)
+        self.faces = [None] * P
+        self.scal = [None] * P
+        self.tmp = [None] * P
+
+    def view(self, r):
+        ring = self
+
+        class View:
+            world, rank = ring.P, r
+            below, above = (r - 1) % ring.P, (r + 1) % ring.P
+
+            def start(self, send_lo, send_hi, recv_lo, recv_hi):
+                ring.faces[r] = (send_lo, send_hi)
+                main, cur = torch.cuda.default_stream(), torch.cuda.current_stream()
+                ring.barrier.wait()                      # every rank's pack kernel is enqueued on the main stream
+                cur.wait_stream(main)                    # (the communicator calls this on its own side stream)
+                recv_hi.copy_(ring.faces[self.above][0])
+                recv_lo.copy_(ring.faces[self.below][1])
+                main.wait_stream(cur)                    # nobody's next pack may overtake these copies
+                ring.barrier.wait()                      # every copy is enqueued before anyone packs again
+                return []
+
+            @staticmethod
+            def finish(reqs):
+                pass
+
+            def __call__(self, *a):
+                self.finish(self.start(*a))
+
+            def allreduce_sum(self, t):
+                ring.scal[r] = t
+                ring.barrier.wait()
+                acc = ring.scal[0].clone()
+                for k in range(1, ring.P):               # same order on every rank: identical bits everywhere
+                    acc += ring.scal[k]
+                ring.tmp[r] = acc
+                ring.barrier.wait()
+                t.copy_(acc)
+                ring.barrier.wait()
+                return t
+
+        return View()
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("L,P,theta", [((8, 4, 4, 8), 2, (0, 0, 0, np.pi)), ((4, 4, 4, 12), 3, None), ((4, 4, 4, 8), 1, None)])
+def test_cg_over_slabs(L, P, theta):
+    """lqcd_cg_solve_slab on P slabs (P threads, one per 'rank', all calling the library together as P processes
+    would) against the oracle's CG on the whole lattice: solution, iteration count, residuals."""
+    import threading
+
+    kappa, csw = 0.125, 1.0
+    U = synth.smooth_gauge(L, 111)
+    b = synth.gaussian_spinor(L, 112)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, B.F64, B.RECON_18) for r in range(P)]
+    ring = ThreadRing(P)
+    out = np.empty_like(b)
+    infos, errors = [None] * P, []
+
+    def run(r):
+        try:
+            R = ranks[r]
+            B.spinor_import(R.g, to_dev(b[R.lo:R.hi]), R.src, B.F64)
+            comm = slab.SlabCommunicator(R.g, ring.view(r))
+            ws = B.alloc_field(R.g, B.FIELD_WORKSPACE)
+            infos[r] = slab.cg_solve_slab(R.g, kappa, R.U, R.A, R.src, R.dst, ws, comm, tol=1e-10, maxiter=4000)
+            o = torch.empty((R.hi - R.lo, 4, 3), dtype=torch.complex128, device="cuda")
+            B.spinor_export(R.g, R.dst, o, B.F64)
+            torch.cuda.synchronize()
+            out[R.lo:R.hi] = o.cpu().numpy()
+        except Exception as e:   # noqa: BLE001
+            errors.append(e)
+            ring.barrier.abort()
+
+    threads = [threading.Thread(target=run, args=(r,)) for r in range(P)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(500)
+    assert not errors, errors
+    xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, theta=theta, tol=1e-10)
+    assert np.linalg.norm(out - xo) / np.linalg.norm(xo) <= 1e-8
+    for info in infos:
+        assert info["status"] == B.OK and abs(info["iters"] - it_o) <= 2
+        assert info["rel_resid_normal"] <= 2e-10 and info["rel_resid_true"] <= 1e-8
+        assert info["iters"] == infos[0]["iters"]          # lockstep
+    r = oracle.dw(L, U, out, kappa, A, theta=theta) - b
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1e-8
+    for R in ranks:
+        B.geom_destroy(R.g)

@@ -35,10 +35,10 @@ for t in range(T):
     U[t * ns:(t + 1) * ns] = float(t0 + t)
 halo_lo, halo_hi = slab.gauge_halo_exchange(U, L, xch)
 s = xch.allreduce_sum(torch.tensor([float(rank + 1)], dtype=torch.float64))
-print(json.dumps({"rank": rank, "world": world, "t0": t0, "T": T, "below": xch.below, "above": xch.above,
+open(os.path.join(%r, "rank%%d.json" %% rank), "w").write(json.dumps({"rank": rank, "world": world, "t0": t0, "T": T, "below": xch.below, "above": xch.above,
                   "recv_lo": sorted(set(recv_lo.tolist())), "recv_hi": sorted(set(recv_hi.tolist())),
                   "halo_lo": sorted(set(halo_lo.real.flatten().tolist())),
-                  "halo_hi": sorted(set(halo_hi.real.flatten().tolist())), "sum": s.item()}), flush=True)
+                  "halo_hi": sorted(set(halo_hi.real.flatten().tolist())), "sum": s.item()}))
 dist.barrier()
 dist.destroy_process_group()
 '''
@@ -47,17 +47,16 @@ dist.destroy_process_group()
 @pytest.mark.parametrize("world,port", [(2, 29551), (3, 29552)])
 def test_face_exchange_on_the_time_ring(tmp_path, world, port):
     script = tmp_path / "worker.py"
-    script.write_text(WORKER % ROOT)
+    script.write_text(WORKER % (ROOT, str(tmp_path)))   # every rank writes its own file: stdout lines can interleave
     env = dict(os.environ, MASTER_ADDR="127.0.0.1")
     out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
                           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)],
                          capture_output=True, text=True, timeout=300, env=env)
     assert out.returncode == 0, out.stderr[-2000:]
     rows = {}
-    for l in out.stdout.splitlines():
-        if l.startswith("{"):
-            d = json.loads(l)
-            rows[d["rank"]] = d
+    for r in range(world):
+        d = json.loads((tmp_path / ("rank%d.json" % r)).read_text())
+        rows[d["rank"]] = d
     assert sorted(rows) == list(range(world))
     L4 = 4 * world
     for r, d in rows.items():
