@@ -76,3 +76,53 @@ def test_dw_48x48x48x96_sampled(fields, prec, recon):
         assert err.max() <= TOL[prec], (dagger, err.max())
     del canon, src, dst, A, U
     torch.cuda.empty_cache()
+
+
+def test_slab_decomposition_48x48x48x96_sampled(fields):
+    """NEXT-3 at full size: the lattice as two 48^3 x 48 time slabs (what two ranks would hold), clover term of each
+    slab from lqcd_clover_build_slab with the one-slice gauge halo, pack -> face copies -> pipeline kernel -> face
+    kernel; sampled sites (plus 256 on each of the four face slices) against the oracle on the whole lattice."""
+    from paper_2503_16994_b200 import slab
+
+    P, V = 2, synth.vol(L)
+    ns, T = L[0] * L[1] * L[2], L[3] // P
+    Uc, psic = fields["Uc"], fields["psic"]
+    rng = np.random.Generator(np.random.PCG64(synth.seed_for(5, 8)))
+    face = np.concatenate([t * ns + rng.integers(0, ns, size=256) for t in (0, T - 1, T, L[3] - 1)])
+    sites = np.array(sorted(set(int(s) for s in np.concatenate([sample_sites(), face]))), dtype=np.int64)
+    ranks = []
+    for r in range(P):
+        g = slab.slab_geom_create(L, P, None)
+        assert "dw_pipe_kernel" in B.dw_plan(g, B.F64, B.RECON_18, True)
+        lo, hi = r * T * ns, (r + 1) * T * ns
+        U = B.alloc_field(g, B.FIELD_GAUGE)
+        B.gauge_import(g, Uc[lo:hi], U)
+        below = Uc[((lo - ns) % V):((lo - ns) % V) + ns].contiguous()
+        above = Uc[(hi % V):(hi % V) + ns].contiguous()
+        A = B.alloc_field(g, B.FIELD_CLOVER)
+        B.clover_build_slab(g, KAPPA, CSW, U, below, above, A)
+        src, dst = B.alloc_field(g, B.FIELD_SPINOR), B.alloc_field(g, B.FIELD_SPINOR)
+        B.spinor_import(g, psic[lo:hi], src)
+        faces = [B.alloc_field(g, B.FIELD_FACE) for _ in range(4)]   # send_lo, send_hi, recv_lo, recv_hi
+        ranks.append(dict(g=g, U=U, A=A, src=src, dst=dst, f=faces, lo=lo, hi=hi))
+    canon = torch.empty((V, 4, 3), dtype=torch.complex128, device="cuda")
+    for dagger, fn in ((False, B.dw_apply), (True, B.dwdag_apply)):
+        for R in ranks:
+            B.dw_slab_pack(R["g"], KAPPA, R["U"], R["src"], R["f"][0], R["f"][1], dagger)
+        for r, R in enumerate(ranks):
+            ranks[(r - 1) % P]["f"][3].copy_(R["f"][0])
+            ranks[(r + 1) % P]["f"][2].copy_(R["f"][1])
+        for R in ranks:
+            R["dst"].fill_(0x7F)
+            fn(R["g"], KAPPA, R["U"], R["A"], R["src"], R["dst"])
+            B.dw_slab_faces(R["g"], KAPPA, R["U"], R["f"][2], R["f"][3], R["dst"], dagger)
+            B.spinor_export(R["g"], R["dst"], canon[R["lo"]:R["hi"]])
+        torch.cuda.synchronize()
+        got = canon[torch.from_numpy(sites).cuda()].cpu().numpy()
+        ref = oracle.dw_at_sites(L, fields["U_host"], fields["psi_host"], sites, KAPPA, CSW, dagger=dagger)
+        err = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(ref.reshape(len(sites), -1), axis=1)
+        assert err.max() <= 1e-12, (dagger, err.max())
+    for R in ranks:
+        B.geom_destroy(R["g"])
+    del ranks, canon
+    torch.cuda.empty_cache()
