@@ -185,24 +185,26 @@ lqcd_status lqcd_clover_build_slab(const lqcd_geom* g, const lqcd_dirac* d, cons
  * product summed over the ranks.  All ranks call it together with their slab's fields.  The library does no
  * communication itself: the caller supplies three host callbacks, each called while the library enqueues work on
  * `stream`, each returning 0 on success (nonzero aborts the solve with LQCD_ECUDA on that rank):
- *   exchange_start(ctx): send_lo / send_hi have been written by work already enqueued on `stream`; start moving send_lo
- *                        into the rank below's recv_hi and send_hi into the rank above's recv_lo (ordered after
- *                        `stream`'s current tail, e.g. on a second stream so that it overlaps the stencil kernel);
+ *   exchange_start(ctx, nbytes): the first nbytes of send_lo / send_hi have been written by work already enqueued on
+ *                        `stream`; start moving them into the rank below's recv_hi and the rank above's recv_lo
+ *                        (ordered after `stream`'s current tail, e.g. on a second stream so that the transfer overlaps
+ *                        the stencil kernel).  nbytes = lqcd_field_bytes(LQCD_FIELD_FACE) of the precision at work;
  *   exchange_wait(ctx) : make `stream` wait until recv_lo / recv_hi have arrived;
  *   allreduce_sum(ctx, n): sum scalars[0..n) (DEVICE doubles, written by work enqueued on `stream`) over all ranks,
  *                        in place, ordered on `stream`.
- * Face buffers and scalars (>= 4 doubles): DEVICE, caller-owned.  b, x: this rank's slab of the source / solution.
- * info as lqcd_cg_solve (the residuals are those of the whole lattice).  parm->mixed and parm->eo must be 0. */
+ * Face buffers (fp64-sized) and scalars (>= 4 doubles): DEVICE, caller-owned.  b, x: this rank's slab of the source /
+ * solution.  f, parm, info as lqcd_cg_solve (residuals of the whole lattice); parm->mixed != 0 runs the fp32 inner CG
+ * on the slabs too (fp32 faces, half the bytes); parm->eo must be 0. */
 typedef struct {
   void* send_lo; void* send_hi; void* recv_lo; void* recv_hi;
   double* scalars;
-  int (*exchange_start)(void* ctx);
+  int (*exchange_start)(void* ctx, size_t nbytes);
   int (*exchange_wait)(void* ctx);
   int (*allreduce_sum)(void* ctx, int n);
   void* ctx;
 } lqcd_slab_comm;
-lqcd_status lqcd_cg_solve_slab(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, const void* clover64,
-                               const void* b, void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
+lqcd_status lqcd_cg_solve_slab(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b, void* x,
+                               void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
                                const lqcd_slab_comm* comm, lqcd_recon recon, void* stream);
 
 /* SURVEY.md 8(f) NEXT-1 (the 12 colour-spin sources of propagator! share one gauge field): D or D^+

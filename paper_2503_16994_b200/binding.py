@@ -248,22 +248,23 @@ def cg_solve(g, kappa, U64, clover64, b, x, workspace, tol=1e-10, maxiter=10000,
 
 SLAB_CALLBACK = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
 SLAB_CALLBACK_N = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int)
+SLAB_CALLBACK_BYTES = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t)
 
 
 class SlabComm(ctypes.Structure):
     """lqcd_slab_comm: face buffers, the all-reduce payload and the three host callbacks."""
     _fields_ = [("send_lo", ctypes.c_void_p), ("send_hi", ctypes.c_void_p), ("recv_lo", ctypes.c_void_p),
-                ("recv_hi", ctypes.c_void_p), ("scalars", ctypes.c_void_p), ("exchange_start", SLAB_CALLBACK),
+                ("recv_hi", ctypes.c_void_p), ("scalars", ctypes.c_void_p), ("exchange_start", SLAB_CALLBACK_BYTES),
                 ("exchange_wait", SLAB_CALLBACK), ("allreduce_sum", SLAB_CALLBACK_N), ("ctx", ctypes.c_void_p)]
 
 
-def cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, comm, tol=1e-10, maxiter=10000, check_every=16,
-                  recon=RECON_18, stream=None, raise_on_notconv=True, mu=0.0):
-    """lqcd_cg_solve_slab; comm: a SlabComm (paper_2503_16994_b200.slab.make_comm builds one)."""
+def cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, comm, tol=1e-10, maxiter=10000, U32=None, clover32=None,
+                  mixed=False, inner_tol=1e-4, check_every=16, recon=RECON_18, stream=None, raise_on_notconv=True, mu=0.0):
+    """lqcd_cg_solve_slab; comm: a SlabComm (paper_2503_16994_b200.slab.SlabCommunicator builds one)."""
     d = _dirac(kappa, mu=mu)
-    p = CgParm(float(tol), int(maxiter), 0, 0, 1e-4, int(check_every))
+    f, p = _cg_args(U64, clover64, None, U32, clover32, None, tol, maxiter, mixed, False, inner_tol, check_every)
     info = CgInfo()
-    st = lib().lqcd_cg_solve_slab(g, ctypes.byref(d), _ptr(U64), _ptr(clover64), _ptr(b), _ptr(x), _ptr(workspace),
+    st = lib().lqcd_cg_solve_slab(g, ctypes.byref(d), ctypes.byref(f), _ptr(b), _ptr(x), _ptr(workspace),
                                   ctypes.byref(p), ctypes.byref(info), ctypes.byref(comm), recon, _stream(stream))
     if st != OK and not (st == ENOTCONV and not raise_on_notconv):
         _check(st)

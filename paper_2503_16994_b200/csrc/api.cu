@@ -705,6 +705,9 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
 
 // ---- NEXT-3: CG over the time slabs of a decomposed lattice -------------------------------------------------------
 namespace {
+#define LSS(e) do { lqcd_status _st = (e); if (_st != LQCD_OK) return _st; } while (0)
+
+template <typename T>
 struct SlabSolve {
   const lqcd_geom* h;
   const lqcd_dirac* d;
@@ -715,21 +718,20 @@ struct SlabSolve {
   double* partial;
   cudaStream_t s;
 
+  size_t face_bytes() const { return (size_t)h->g.L[0] * h->g.L[1] * h->g.L[2] * 6 * 2 * sizeof(T); }
   lqcd_status cb(int rc, const char* what) const {
     if (rc != 0) { set_error("lqcd_cg_solve_slab: callback %s failed (%d)", what, rc); return LQCD_ECUDA; }
     return LQCD_OK;
   }
   // out = D in (D^+ in) on this rank's slab, faces included
   lqcd_status apply(const void* in, void* out, bool dagger) const {
-    CKS(slab_pack<double>(h, dagger, U, recon, in, comm->send_lo, comm->send_hi, s), "slab_pack");
-    lqcd_status st = cb(comm->exchange_start(comm->ctx), "exchange_start");
-    if (st != LQCD_OK) return st;
-    Op<double> M;
+    CKS(slab_pack<T>(h, dagger, U, recon, in, comm->send_lo, comm->send_hi, s), "slab_pack");
+    LSS(cb(comm->exchange_start(comm->ctx, face_bytes()), "exchange_start"));
+    Op<T> M;
     M.geom = h; M.U = U; M.A = A; M.Ainv = nullptr; M.tmp = nullptr; M.kappa = d->kappa; M.mu = d->mu; M.recon = recon; M.eo = false;
     CKS(M.apply(in, out, dagger, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "slab stencil");
-    st = cb(comm->exchange_wait(comm->ctx), "exchange_wait");
-    if (st != LQCD_OK) return st;
-    CKS(slab_faces<double>(h, d->kappa, dagger, U, recon, comm->recv_lo, comm->recv_hi, out, s), "slab_faces");
+    LSS(cb(comm->exchange_wait(comm->ctx), "exchange_wait"));
+    CKS(slab_faces<T>(h, d->kappa, dagger, U, recon, comm->recv_lo, comm->recv_hi, out, s), "slab_faces");
     return LQCD_OK;
   }
   // scalars[0] = sum over ranks of the `nblocks` partial sums in `partial`
@@ -738,28 +740,65 @@ struct SlabSolve {
     return cb(comm->allreduce_sum(comm->ctx, 1), "allreduce_sum");
   }
   lqcd_status norm2(const void* v, size_t n, double* host) const {
-    CKS(norm2_partial<double>(v, n, partial, s), "norm2");
-    lqcd_status st = reduce(reduce_blocks(n));
-    if (st != LQCD_OK) return st;
+    CKS(norm2_partial<T>(v, n, partial, s), "norm2");
+    LSS(reduce(reduce_blocks(n)));
     if (host) {
       CKS(cudaMemcpyAsync(host, comm->scalars, sizeof(double), cudaMemcpyDeviceToHost, s), "copy scalar");
       CKS(cudaStreamSynchronize(s), "sync");
     }
     return LQCD_OK;
   }
+  // CG on D^+D x = bp from x = 0 (the algorithm of cg_normal; unfused residual update, all-reduced scalars).
+  // Every rank sees the same all-reduced scalars, hence the same state: the ranks stay in lockstep.
+  lqcd_status cg(const void* bp, void* x, void* r, void* p, void* t, void* q, CgState* state, double tol, int maxiter,
+                 int check, CgState* hs) const {
+    typedef typename vec2<T>::type T2;
+    const size_t n = spinor_complex(h->g);
+    const size_t bytes = n * sizeof(T2);
+    CKS(cudaMemsetAsync(x, 0, bytes, s), "memset");
+    CKS(cudaMemcpyAsync(r, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+    CKS(cudaMemcpyAsync(p, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+    LSS(norm2(r, n, nullptr));
+    CKS(cg_init_state(state, comm->scalars, 1, tol, s), "cg_init_state");
+    int launched = 0;
+    for (;;) {
+      CKS(cudaMemcpyAsync(hs, state, sizeof(CgState), cudaMemcpyDeviceToHost, s), "copy state");
+      CKS(cudaStreamSynchronize(s), "sync");
+      if (hs->done || launched >= maxiter) break;
+      int batch = check;
+      if (launched + batch > maxiter) batch = maxiter - launched;
+      for (int it = 0; it < batch; it++) {
+        LSS(apply(p, t, false));
+        CKS(norm2_partial<T>(t, n, partial, s), "norm2");
+        LSS(reduce(reduce_blocks(n)));
+        CKS(cg_reduce_alpha(state, comm->scalars, 1, s), "alpha");
+        LSS(apply(t, q, true));
+        CKS(cg_raxpy_norm<T>(state, q, r, n, partial, s), "r -= alpha q");
+        LSS(reduce(reduce_blocks(n)));
+        CKS(cg_reduce_beta(state, comm->scalars, 1, s), "beta");
+        CKS(cg_update_xp<T>(state, x, p, r, n, s), "update");
+      }
+      launched += batch;
+    }
+    return LQCD_OK;
+  }
 };
-#define LSS(e) do { lqcd_status _st = (e); if (_st != LQCD_OK) return _st; } while (0)
 }  // namespace
 
-extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, const void* clover64,
-                                          const void* b, void* x, void* workspace, const lqcd_cg_parm* parm,
-                                          lqcd_cg_info* info, const lqcd_slab_comm* comm, lqcd_recon recon, void* stream) {
-  REQUIRE(h && d && U64 && b && x && workspace && parm && info && comm, "lqcd_cg_solve_slab: NULL argument");
+extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b,
+                                          void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
+                                          const lqcd_slab_comm* comm, lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && f && b && x && workspace && parm && info && comm, "lqcd_cg_solve_slab: NULL argument");
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_cg_solve_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
   REQUIRE(valid_recon(recon), "lqcd_cg_solve_slab: bad recon");
+  REQUIRE(f->U64, "lqcd_cg_solve_slab: U64 is required");
   REQUIRE(x != b, "lqcd_cg_solve_slab: x aliases b");
   REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve_slab: bad tol / maxiter");
-  REQUIRE(!parm->mixed && !parm->eo, "lqcd_cg_solve_slab: plain fp64 CG only (mixed and eo must be 0)");
+  REQUIRE(!parm->eo, "lqcd_cg_solve_slab: the even-odd operator is not available on slabs (eo must be 0)");
+  if (parm->mixed) {
+    REQUIRE(f->U32, "lqcd_cg_solve_slab: mixed needs U32");
+    REQUIRE((f->clover64 == nullptr) == (f->clover32 == nullptr), "lqcd_cg_solve_slab: mixed needs clover32 iff clover64");
+  }
   REQUIRE(comm->send_lo && comm->send_hi && comm->recv_lo && comm->recv_hi && comm->scalars, "lqcd_cg_solve_slab: NULL comm buffer");
   REQUIRE(comm->exchange_start && comm->exchange_wait && comm->allreduce_sum, "lqcd_cg_solve_slab: NULL callback");
   memset(info, 0, sizeof(*info));
@@ -768,47 +807,57 @@ extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* 
   cudaStream_t s = as_stream(stream);
   Workspace ws{(char*)workspace, 0};
   const size_t sites = (size_t)2 * g.Vh;
-  void* v64[WS_SPINORS64];
+  void *v64[WS_SPINORS64], *v32[WS_SPINORS32];
   for (int i = 0; i < WS_SPINORS64; i++) v64[i] = ws.take(sites * 12 * sizeof(double2));
-  for (int i = 0; i < WS_SPINORS32; i++) ws.take(sites * 12 * sizeof(float2));
+  for (int i = 0; i < WS_SPINORS32; i++) v32[i] = ws.take(sites * 12 * sizeof(float2));
   double* partial = (double*)ws.take(partial_len(g) * sizeof(double));
   ws.take(64);
   CgState* state = (CgState*)ws.take(sizeof(CgState));
   const size_t n = spinor_complex(g);
-  const size_t bytes = n * sizeof(double2);
-  SlabSolve S{h, d, U64, clover64, (int)recon, comm, partial, s};
+  SlabSolve<double> S{h, d, f->U64, f->clover64, (int)recon, comm, partial, s};
   void *r = v64[0], *p = v64[1], *t = v64[2], *q = v64[3], *bp = v64[4];
-
-  LSS(S.apply(b, bp, true));                                   // b' = D^+ b
-  CKS(cudaMemsetAsync(x, 0, bytes, s), "memset");
-  CKS(cudaMemcpyAsync(r, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
-  CKS(cudaMemcpyAsync(p, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
-  LSS(S.norm2(r, n, nullptr));
-  CKS(cg_init_state(state, comm->scalars, 1, parm->tol, s), "cg_init_state");
   const int check = parm->check_every > 0 ? parm->check_every : 16;
   CgState hs;
-  int launched = 0;
-  for (;;) {   // every rank sees the same all-reduced scalars, hence the same state: the ranks stay in lockstep
-    CKS(cudaMemcpyAsync(&hs, state, sizeof(CgState), cudaMemcpyDeviceToHost, s), "copy state");
-    CKS(cudaStreamSynchronize(s), "sync");
-    if (hs.done || launched >= parm->maxiter) break;
-    int batch = check;
-    if (launched + batch > parm->maxiter) batch = parm->maxiter - launched;
-    for (int it = 0; it < batch; it++) {
-      LSS(S.apply(p, t, false));
-      CKS(norm2_partial<double>(t, n, partial, s), "norm2");
-      LSS(S.reduce(reduce_blocks(n)));
-      CKS(cg_reduce_alpha(state, comm->scalars, 1, s), "alpha");
+  memset(&hs, 0, sizeof(hs));
+  double rho0 = 0;
+  bool converged = false;
+
+  LSS(S.apply(b, bp, true));                                   // b' = D^+ b
+  if (!parm->mixed) {
+    LSS(S.cg(bp, x, r, p, t, q, state, parm->tol, parm->maxiter, check, &hs));
+    info->iters = hs.iters;
+    rho0 = hs.rho0;
+    if (hs.breakdown) { set_error("lqcd_cg_solve_slab: breakdown (NaN or <p,D^+D p> <= 0) at iteration %d", hs.iters); return LQCD_EBREAKDOWN; }
+    converged = hs.done != 0;
+  } else {
+    // defect correction as in lqcd_cg_solve: r = b' - D^+D x (fp64); e = CG32(r) to inner_tol; x += e
+    SlabSolve<float> S32{h, d, f->U32, f->clover32, (int)recon, comm, partial, s};
+    double rho = 0;
+    int total = 0;
+    const double inner_tol = parm->inner_tol > 0 ? parm->inner_tol : 1e-4;
+    CKS(cudaMemsetAsync(x, 0, n * sizeof(double2), s), "memset");
+    CKS(cudaMemcpyAsync(r, bp, n * sizeof(double2), cudaMemcpyDeviceToDevice, s), "copy");
+    LSS(S.norm2(r, n, &rho0));
+    rho = rho0;
+    for (;;) {
+      if (rho0 == 0.0 || rho <= parm->tol * parm->tol * rho0) { converged = true; break; }
+      if (!(rho == rho)) { info->iters = total; set_error("lqcd_cg_solve_slab: NaN residual in mixed solve"); return LQCD_EBREAKDOWN; }
+      if (total >= parm->maxiter) break;
+      CKS(to_f32(r, v32[0], n, s), "to_f32");
+      const double need = parm->tol * sqrt(rho0 / rho) * 0.5;
+      const double itol = inner_tol > need ? inner_tol : need;
+      LSS(S32.cg(v32[0], v32[5], v32[1], v32[2], v32[3], v32[4], state, itol, parm->maxiter - total, check, &hs));
+      total += hs.iters;
+      info->outer += 1;
+      if (hs.breakdown) { info->iters = total; set_error("lqcd_cg_solve_slab: breakdown in the fp32 inner solve"); return LQCD_EBREAKDOWN; }
+      CKS(add_f32_to_f64(v32[5], x, n, s), "x += e");
+      LSS(S.apply(x, t, false));
       LSS(S.apply(t, q, true));
-      CKS(cg_raxpy_norm<double>(state, q, r, n, partial, s), "r -= alpha q");
-      LSS(S.reduce(reduce_blocks(n)));
-      CKS(cg_reduce_beta(state, comm->scalars, 1, s), "beta");
-      CKS(cg_update_xp<double>(state, x, p, r, n, s), "update");
+      CKS(xmy<double>(bp, q, r, n, s), "r = b' - q");
+      LSS(S.norm2(r, n, &rho));
     }
-    launched += batch;
+    info->iters = total;
   }
-  info->iters = hs.iters;
-  if (hs.breakdown) { set_error("lqcd_cg_solve_slab: breakdown (NaN or <p,D^+D p> <= 0) at iteration %d", hs.iters); return LQCD_EBREAKDOWN; }
   // true residuals with fresh operator applications (R11), norms over the whole lattice
   double nb = 0, nr = 0, nq = 0;
   LSS(S.apply(x, t, false));
@@ -818,9 +867,9 @@ extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* 
   LSS(S.apply(t, q, true));
   LSS(S.norm2(q, n, &nq));
   info->rel_resid_true = nb > 0 ? sqrt(nr / nb) : 0.0;
-  info->rel_resid_normal = hs.rho0 > 0 ? sqrt(nq / hs.rho0) : 0.0;
+  info->rel_resid_normal = rho0 > 0 ? sqrt(nq / rho0) : 0.0;
   info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
-  if (!hs.done) { set_error("lqcd_cg_solve_slab: not converged after %d iterations", hs.iters); return LQCD_ENOTCONV; }
+  if (!converged) { set_error("lqcd_cg_solve_slab: not converged after %d iterations", info->iters); return LQCD_ENOTCONV; }
   return LQCD_OK;
 }
 

@@ -160,10 +160,10 @@ class SlabCommunicator:
                     return 1
             return wrapper
 
-        def start(_ctx):
+        def start(_ctx, nbytes):   # fp32 faces use the first half of the buffers
             self.comm_stream.wait_stream(torch.cuda.current_stream())
             with torch.cuda.stream(self.comm_stream):
-                xch.finish(xch.start(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi))
+                xch.finish(xch.start(self.send_lo[:nbytes], self.send_hi[:nbytes], self.recv_lo[:nbytes], self.recv_hi[:nbytes]))
 
         def wait(_ctx):
             torch.cuda.current_stream().wait_stream(self.comm_stream)
@@ -172,7 +172,7 @@ class SlabCommunicator:
             xch.allreduce_sum(self.scalars[:n])
 
         # keep the CFUNCTYPE objects alive as long as the struct
-        self._cbs = (B.SLAB_CALLBACK(guarded(start)), B.SLAB_CALLBACK(guarded(wait)), B.SLAB_CALLBACK_N(guarded(allreduce)))
+        self._cbs = (B.SLAB_CALLBACK_BYTES(guarded(start)), B.SLAB_CALLBACK(guarded(wait)), B.SLAB_CALLBACK_N(guarded(allreduce)))
         self.struct = B.SlabComm(self.send_lo.data_ptr(), self.send_hi.data_ptr(), self.recv_lo.data_ptr(),
                                  self.recv_hi.data_ptr(), self.scalars.data_ptr(), self._cbs[0], self._cbs[1],
                                  self._cbs[2], ctypes.c_void_p(None))
