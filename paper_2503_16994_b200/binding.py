@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(HERE, "liblqcd_b200.so")
 OK, EINVAL, ENOMEM, ECUDA, ENOTCONV, EBREAKDOWN, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB, BC_SLAB = 0, 1, 2, 3, 4
 F64, F32 = 0, 1
+SLAB_OPEN_LO, SLAB_OPEN_HI = 1, 2
 RECON_18, RECON_12 = 18, 12
 FIELD_GAUGE, FIELD_SPINOR, FIELD_CLOVER, FIELD_WORKSPACE, FIELD_FACE = 0, 1, 2, 3, 4
 
@@ -36,7 +37,8 @@ class LqcdError(RuntimeError):
 
 class GeomDesc(ctypes.Structure):
     _fields_ = [("L", ctypes.c_int * 4), ("bc", ctypes.c_int), ("theta", ctypes.c_double * 4),
-                ("phi0", ctypes.c_double * 3), ("phiT", ctypes.c_double * 3), ("device", ctypes.c_int)]
+                ("phi0", ctypes.c_double * 3), ("phiT", ctypes.c_double * 3), ("device", ctypes.c_int),
+                ("slab_edges", ctypes.c_int)]
 
 
 class Dirac(ctypes.Structure):
@@ -108,7 +110,7 @@ def _dirac(kappa, csw=0.0, ct=1.0, mu=0.0):
     return Dirac(float(kappa), float(csw), float(ct), float(mu))
 
 
-def geom_desc(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0):
+def geom_desc(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0, slab_edges=0):
     d = GeomDesc()
     for i in range(4):
         d.L[i] = int(L[i])
@@ -118,11 +120,12 @@ def geom_desc(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0):
         d.phi0[i] = float(phi0[i]) if phi0 is not None else 0.0
         d.phiT[i] = float(phiT[i]) if phiT is not None else 0.0
     d.device = int(device)
+    d.slab_edges = int(slab_edges)
     return d
 
 
-def geom_create(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0):
-    d = geom_desc(L, bc, theta, phi0, phiT, device)
+def geom_create(L, bc=BC_PERIODIC, theta=None, phi0=None, phiT=None, device=0, slab_edges=0):
+    d = geom_desc(L, bc, theta, phi0, phiT, device, slab_edges)
     g = ctypes.c_void_p()
     _check(lib().lqcd_geom_create(ctypes.byref(d), ctypes.byref(g)))
     return g
@@ -179,9 +182,10 @@ def clover_build(g, kappa, csw, U64, clover, clover_inv=None, recon=RECON_18, ou
 
 
 def clover_build_slab(g, kappa, csw, U64, halo_lo, halo_hi, clover, clover_inv=None, recon=RECON_18, out_prec=F64,
-                      stream=None):
-    """Csw! on a time slab (BC_SLAB); halo_lo / halo_hi: the neighbour ranks' adjacent time slices, canonical fp64."""
-    d = _dirac(kappa, csw)
+                      stream=None, ct=1.0):
+    """Csw! on a time slab (BC_SLAB); halo_lo / halo_hi: the neighbour ranks' adjacent time slices, canonical fp64
+    (None on a face that is an open boundary)."""
+    d = _dirac(kappa, csw, ct)
     _check(lib().lqcd_clover_build_slab(g, ctypes.byref(d), _ptr(U64), recon, _ptr(halo_lo), _ptr(halo_hi), _ptr(clover),
                                         _ptr(clover_inv), out_prec, _stream(stream)))
 

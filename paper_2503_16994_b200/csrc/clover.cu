@@ -263,9 +263,10 @@ __global__ void __launch_bounds__(CLV_THREADS, CLV_MINB) clover_kernel(const Clo
   }
   double dadd = 0.0;
   if (!fz && g.bc != LQCD_BC_PERIODIC && cp.ct != 1.0) {  // R10: + 2 kappa (ct - 1) next to the frozen slices
-    const int last = (g.bc == LQCD_BC_OPEN) ? g.L[3] - 2 : g.L[3] - 1;
-    if (x3 == 1) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
-    if (x3 == last) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
+    const bool slab = g.bc == LQCD_BC_SLAB;   // a slab has the term only next to its open faces
+    const int last = (g.bc == LQCD_BC_OPEN || slab) ? g.L[3] - 2 : g.L[3] - 1;
+    if (x3 == 1 && (!slab || (g.edges & LQCD_SLAB_OPEN_LO))) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
+    if (x3 == last && (!slab || (g.edges & LQCD_SLAB_OPEN_HI))) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
   }
   const size_t TV = g.TV;
 #pragma unroll 1

@@ -29,6 +29,7 @@ struct Geom {
   int TV;         // sites of one parity per tile
   int ntiles;
   int bc;         // lqcd_bc
+  int edges;      // LQCD_BC_SLAB: LQCD_SLAB_OPEN_LO | LQCD_SLAB_OPEN_HI (faces that are open boundaries of the lattice)
   long long Vh;   // sites of one parity
   // device table, TILE_TAB ints per tile: linear index of the 8 neighbour tiles (2*mu + (0: +mu, 1: -mu)),
   // then the time coordinate of the tile origin (library-owned, built by lqcd_geom_create)
@@ -83,6 +84,7 @@ __host__ __device__ inline void site_locate(const Geom& g, const int x[4], int& 
 __host__ __device__ inline bool frozen_slice(const Geom& g, int x3) {
   if (g.bc == LQCD_BC_OPEN) return x3 == 0 || x3 == g.L[3] - 1;
   if (g.bc == LQCD_BC_SF_ORBI || g.bc == LQCD_BC_SF_AFWB) return x3 == 0;
+  if (g.bc == LQCD_BC_SLAB) return ((g.edges & LQCD_SLAB_OPEN_LO) && x3 == 0) || ((g.edges & LQCD_SLAB_OPEN_HI) && x3 == g.L[3] - 1);
   return false;
 }
 
@@ -90,7 +92,7 @@ __host__ __device__ inline bool frozen_slice(const Geom& g, int x3) {
 // open / SF: hops onto frozen slices (D7).  Slab: hops across the slab's two time
 // faces -- the face kernels of slab.cu add them from the exchanged half spinors.
 __host__ __device__ inline bool time_hop_blocked(const Geom& g, int x3, bool fwd) {
-  if (g.bc == LQCD_BC_SLAB) return fwd ? (x3 + 1 == g.L[3]) : (x3 == 0);
+  if (g.bc == LQCD_BC_SLAB && (fwd ? (x3 + 1 == g.L[3]) : (x3 == 0))) return true;
   const int xn = fwd ? ((x3 + 1 == g.L[3]) ? 0 : x3 + 1) : ((x3 == 0) ? g.L[3] - 1 : x3 - 1);
   return frozen_slice(g, xn);
 }

@@ -34,46 +34,69 @@ def slab_theta(theta, L4, world):
     return th
 
 
-def ring_neighbours(world, rank):
-    """(rank below, rank above) on the periodic time ring."""
-    return (rank - 1) % world, (rank + 1) % world
+def ring_neighbours(world, rank, periodic=True):
+    """(rank below, rank above) along time; None across an open boundary of the lattice."""
+    below, above = (rank - 1) % world, (rank + 1) % world
+    if not periodic:
+        below = None if rank == 0 else below
+        above = None if rank == world - 1 else above
+    return below, above
 
 
-def slab_geom_create(L, world, theta=None, device=0):
-    """Geometry handle of one rank's slab of the lattice L (periodic in time; antiperiodic = theta4 = pi)."""
+def slab_edges(world, rank, bc=B.BC_PERIODIC):
+    """lqcd_geom_desc.slab_edges of this rank: which of its faces are open boundaries of the lattice."""
+    if bc == B.BC_PERIODIC:
+        return 0
+    if bc != B.BC_OPEN:
+        raise ValueError("only lattices periodic or open in time are decomposed (bc=%r)" % (bc,))
+    return (B.SLAB_OPEN_LO if rank == 0 else 0) | (B.SLAB_OPEN_HI if rank == world - 1 else 0)
+
+
+def slab_geom_create(L, world, theta=None, device=0, rank=0, bc=B.BC_PERIODIC):
+    """Geometry handle of one rank's slab of the lattice L (bc: periodic in time -- antiperiodic = theta4 = pi -- or
+    open, in which case the first and last rank get a frozen outer slice)."""
     T = slab_extent(L[3], world)
-    return B.geom_create((L[0], L[1], L[2], T), B.BC_SLAB, slab_theta(theta, L[3], world), device=device)
+    return B.geom_create((L[0], L[1], L[2], T), B.BC_SLAB, slab_theta(theta, L[3], world), device=device,
+                         slab_edges=slab_edges(world, rank, bc))
 
 
 class FaceExchange:
     """send_lo -> the rank below (lands in its recv_hi), send_hi -> the rank above (lands in its recv_lo).
 
-    world == 1: the slab is its own neighbour on both sides (the periodic lattice).  Tensors of any device / dtype;
-    the two directions carry different tags so that world == 2 (both neighbours are the same peer) cannot mix them.
+    world == 1, periodic: the slab is its own neighbour on both sides (the periodic lattice).  periodic=False (open
+    lattice): the first rank has nobody below, the last nobody above; those faces are left alone.  Tensors of any
+    device / dtype; the two directions carry different tags so that world == 2 (both neighbours are the same peer)
+    cannot mix them.
     """
     TAG_DOWN, TAG_UP = 11, 12
 
-    def __init__(self, group=None):
+    def __init__(self, group=None, periodic=True):
         import torch.distributed as dist
 
         self.dist = dist
         self.group = group
+        self.periodic = periodic
         active = dist.is_available() and dist.is_initialized()
         self.world = dist.get_world_size(group) if active else 1
         self.rank = dist.get_rank(group) if active else 0
-        self.below, self.above = ring_neighbours(self.world, self.rank)
+        self.below, self.above = ring_neighbours(self.world, self.rank, periodic)
 
     def start(self, send_lo, send_hi, recv_lo, recv_hi):
         if self.world == 1:
-            recv_hi.copy_(send_lo)
-            recv_lo.copy_(send_hi)
+            if self.periodic:
+                recv_hi.copy_(send_lo)
+                recv_lo.copy_(send_hi)
             return []
         d = self.dist
-        ops = [d.P2POp(d.isend, send_lo, self.below, self.group, self.TAG_DOWN),
-               d.P2POp(d.isend, send_hi, self.above, self.group, self.TAG_UP),
-               d.P2POp(d.irecv, recv_hi, self.above, self.group, self.TAG_DOWN),
-               d.P2POp(d.irecv, recv_lo, self.below, self.group, self.TAG_UP)]
-        return d.batch_isend_irecv(ops)
+        ops = []
+        if self.below is not None:
+            ops.append(d.P2POp(d.isend, send_lo, self.below, self.group, self.TAG_DOWN))
+        if self.above is not None:
+            ops.append(d.P2POp(d.isend, send_hi, self.above, self.group, self.TAG_UP))
+            ops.append(d.P2POp(d.irecv, recv_hi, self.above, self.group, self.TAG_DOWN))
+        if self.below is not None:
+            ops.append(d.P2POp(d.irecv, recv_lo, self.below, self.group, self.TAG_UP))
+        return d.batch_isend_irecv(ops) if ops else []
 
     @staticmethod
     def finish(reqs):
@@ -119,7 +142,8 @@ def gauge_halo_exchange(U_canon_slab, L, exchange=None):
     """The two time slices the clover builder needs from the ring neighbours (once per configuration).
 
     U_canon_slab: this rank's links, canonical layout [T * L1 L2 L3, 4, 3, 3] complex128 (time slowest).
-    Returns (halo_lo, halo_hi): the slice below the slab's first and the slice above its last."""
+    Returns (halo_lo, halo_hi): the slice below the slab's first and the slice above its last (None across an open
+    boundary)."""
     import torch
 
     xch = exchange if exchange is not None else FaceExchange()
@@ -129,7 +153,8 @@ def gauge_halo_exchange(U_canon_slab, L, exchange=None):
     halo_lo, halo_hi = torch.empty_like(last), torch.empty_like(first)
     # my first slice is the halo_hi of the rank below; my last slice the halo_lo of the rank above
     xch(first, last, halo_lo, halo_hi)
-    return halo_lo, halo_hi
+    # across an open boundary there is no neighbour (and lqcd_clover_build_slab wants no halo there)
+    return (halo_lo if xch.below is not None else None), (halo_hi if xch.above is not None else None)
 
 
 class SlabCommunicator:

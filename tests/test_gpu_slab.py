@@ -29,11 +29,12 @@ def mode(request):
 class Rank:
     """What one rank of the decomposition holds."""
 
-    def __init__(self, L, P, r, theta, U, kappa, csw, prec, recon):
+    def __init__(self, L, P, r, theta, U, kappa, csw, prec, recon, bc=B.BC_PERIODIC, ct=1.0):
         self.T = slab.slab_extent(L[3], P)
         self.ns = L[0] * L[1] * L[2]
         self.lo, self.hi = r * self.T * self.ns, (r + 1) * self.T * self.ns   # canonical site range (time slowest)
-        self.g = slab.slab_geom_create(L, P, theta)
+        self.g = slab.slab_geom_create(L, P, theta, rank=r, bc=bc)
+        self.nbr = slab.ring_neighbours(P, r, bc == B.BC_PERIODIC)
         Uc = to_dev(U[self.lo:self.hi])
         self.U64 = B.alloc_field(self.g, B.FIELD_GAUGE, B.F64, recon)
         B.gauge_import(self.g, Uc, self.U64, B.F64, recon)
@@ -45,7 +46,8 @@ class Rank:
         below = np.arange(self.lo - self.ns, self.lo) % V
         above = np.arange(self.hi, self.hi + self.ns) % V
         self.A = B.alloc_field(self.g, B.FIELD_CLOVER, prec)
-        B.clover_build_slab(self.g, kappa, csw, self.U64, to_dev(U[below]), to_dev(U[above]), self.A, None, recon, prec)
+        B.clover_build_slab(self.g, kappa, csw, self.U64, to_dev(U[below]) if self.nbr[0] is not None else None,
+                            to_dev(U[above]) if self.nbr[1] is not None else None, self.A, None, recon, prec, ct=ct)
         self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (B.alloc_field(self.g, B.FIELD_FACE, prec) for _ in range(4))
         self.src = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
         self.dst = B.alloc_field(self.g, B.FIELD_SPINOR, prec)
@@ -57,9 +59,11 @@ def slab_dw(ranks, kappa, psi, prec, recon, dagger, clover=True, mu=0.0):
         B.spinor_import(R.g, to_dev(psi[R.lo:R.hi]), R.src, prec)
         R.dst.fill_(0x7F)
         B.dw_slab_pack(R.g, kappa, R.U, R.src, R.send_lo, R.send_hi, dagger, prec, recon)
-    for r, R in enumerate(ranks):   # the ring: send_lo -> below's recv_hi, send_hi -> above's recv_lo
-        ranks[(r - 1) % P].recv_hi.copy_(R.send_lo)
-        ranks[(r + 1) % P].recv_lo.copy_(R.send_hi)
+    for R in ranks:   # the ring: send_lo -> below's recv_hi, send_hi -> above's recv_lo (nothing across an open boundary)
+        if R.nbr[0] is not None:
+            ranks[R.nbr[0]].recv_hi.copy_(R.send_lo)
+        if R.nbr[1] is not None:
+            ranks[R.nbr[1]].recv_lo.copy_(R.send_hi)
     out = np.empty_like(psi)
     for R in ranks:
         fn = B.dwdag_apply if dagger else B.dw_apply
@@ -100,6 +104,35 @@ def test_slab_dw_equals_whole_lattice(mode, L, P, theta, prec, recon):
     assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, False, clover=False), ref) <= TOL[prec]
     ref = oracle.dw(L, Uo, psio, kappa, Ao, theta=theta, dagger=True, mu=0.3)
     assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, True, mu=0.3), ref) <= TOL[prec]
+    for R in ranks:
+        B.geom_destroy(R.g)
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
+@pytest.mark.parametrize("L,P", [((8, 4, 4, 8), 2), ((4, 8, 4, 12), 3), ((4, 4, 4, 8), 1), ((6, 4, 4, 8), 2)])
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_slab_dw_open_boundaries(mode, L, P, prec):
+    """A lattice with open time boundaries cut into slabs: the first / last rank carry the frozen slice (D7) and the
+    c~_t term next to it, nothing is exchanged across the open boundary; one slab with both edges open is the open
+    lattice itself.  Against the oracle's open-BC operator on the whole lattice."""
+    kappa, csw, ct, theta, recon = 0.1365, 1.9, 1.2, (0.5, 0.5, 0.5, 0.0), B.RECON_18
+    U = synth.smooth_gauge(L, 121)
+    psi = synth.gaussian_spinor(L, 122)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=B.BC_OPEN, ct=ct)
+    Uo, psio, Ao = (round_f32(U), round_f32(psi), round_f32(A)) if prec == B.F32 else (U, psi, A)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, prec, recon, bc=B.BC_OPEN, ct=ct) for r in range(P)]
+    t = np.arange(psi.shape[0]) // (L[0] * L[1] * L[2])
+    mask = (t >= 1) & (t <= L[3] - 2)
+    for R in ranks:
+        got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
+        B.clover_export(R.g, R.A, got, prec)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+    for dagger in (False, True):
+        ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=B.BC_OPEN, theta=theta, dagger=dagger)
+        got = slab_dw(ranks, kappa, psi, prec, recon, dagger)
+        assert site_rel_err(got, ref, mask) <= TOL[prec]
+        assert np.all(got[~mask] == 0)
     for R in ranks:
         B.geom_destroy(R.g)
 
@@ -158,9 +191,10 @@ class ThreadRing:
     spins on another.
     Same interface and the same who-gets-what as FaceExchange."""
 
-    def __init__(self, P):
+    def __init__(self, P, periodic=True):
         import threading
         self.P = P
+        self.periodic = periodic
         self.barrier = threading.Barrier(P, timeout=120)
         self.faces = [None] * P
         self.scal = [None] * P
@@ -171,15 +205,17 @@ class ThreadRing:
 
         class View:
             world, rank = ring.P, r
-            below, above = (r - 1) % ring.P, (r + 1) % ring.P
+            below, above = slab.ring_neighbours(ring.P, r, ring.periodic)
 
             def start(self, send_lo, send_hi, recv_lo, recv_hi):
                 ring.faces[r] = (send_lo, send_hi)
                 main, cur = torch.cuda.default_stream(), torch.cuda.current_stream()
                 ring.barrier.wait()                      # every rank's pack kernel is enqueued on the main stream
                 cur.wait_stream(main)                    # (the communicator calls this on its own side stream)
-                recv_hi.copy_(ring.faces[self.above][0])
-                recv_lo.copy_(ring.faces[self.below][1])
+                if self.above is not None:
+                    recv_hi.copy_(ring.faces[self.above][0])
+                if self.below is not None:
+                    recv_lo.copy_(ring.faces[self.below][1])
                 main.wait_stream(cur)                    # nobody's next pack may overtake these copies
                 ring.barrier.wait()                      # every copy is enqueued before anyone packs again
                 return []
@@ -208,8 +244,9 @@ class ThreadRing:
 
 @pytest.mark.timeout(600)
 @pytest.mark.parametrize("mixed", [False, True])
-@pytest.mark.parametrize("L,P,theta", [((8, 4, 4, 8), 2, (0, 0, 0, np.pi)), ((4, 4, 4, 12), 3, None), ((4, 4, 4, 8), 1, None)])
-def test_cg_over_slabs(L, P, theta, mixed):
+@pytest.mark.parametrize("L,P,theta,bc", [((8, 4, 4, 8), 2, (0, 0, 0, np.pi), B.BC_PERIODIC), ((4, 4, 4, 12), 3, None, B.BC_PERIODIC),
+                                          ((4, 4, 4, 8), 1, None, B.BC_PERIODIC), ((4, 4, 4, 12), 3, (0.5, 0.5, 0.5, 0), B.BC_OPEN)])
+def test_cg_over_slabs(L, P, theta, bc, mixed):
     """lqcd_cg_solve_slab on P slabs (P threads, one per 'rank', all calling the library together as P processes
     would) against the oracle's CG on the whole lattice: solution, iteration count, residuals."""
     import threading
@@ -217,9 +254,12 @@ def test_cg_over_slabs(L, P, theta, mixed):
     kappa, csw = 0.125, 1.0
     U = synth.smooth_gauge(L, 111)
     b = synth.gaussian_spinor(L, 112)
-    A = oracle.clover_blocks(L, U, kappa, csw)
-    ranks = [Rank(L, P, r, theta, U, kappa, csw, B.F64, B.RECON_18) for r in range(P)]
-    ring = ThreadRing(P)
+    if bc == B.BC_OPEN:   # the solve lives on the interior (D7): a source without support on the frozen slices
+        tt = np.arange(b.shape[0]) // (L[0] * L[1] * L[2])
+        b[(tt == 0) | (tt == L[3] - 1)] = 0
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, B.F64, B.RECON_18, bc=bc) for r in range(P)]
+    ring = ThreadRing(P, periodic=(bc == B.BC_PERIODIC))
     out = np.empty_like(b)
     infos, errors = [None] * P, []
 
@@ -251,14 +291,16 @@ def test_cg_over_slabs(L, P, theta, mixed):
     for t in threads:
         t.join(500)
     assert not errors, errors
-    xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, theta=theta, tol=1e-10)
+    xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, bc=bc, theta=theta, tol=1e-10)
     assert np.linalg.norm(out - xo) / np.linalg.norm(xo) <= 1e-8
     for info in infos:
         assert info["status"] == B.OK and (mixed or abs(info["iters"] - it_o) <= 2)
         assert info["rel_resid_normal"] <= 2e-10 and info["rel_resid_true"] <= 1e-8
         assert (info["outer"] >= 2) == mixed
         assert info["iters"] == infos[0]["iters"]          # lockstep
-    r = oracle.dw(L, U, out, kappa, A, theta=theta) - b
-    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1e-8
+    tt = np.arange(b.shape[0]) // (L[0] * L[1] * L[2])
+    live = (tt >= 1) & (tt <= L[3] - 2) if bc == B.BC_OPEN else np.ones(b.shape[0], dtype=bool)
+    r = (oracle.dw(L, U, out, kappa, A, bc=bc, theta=theta) - b)[live]
+    assert np.linalg.norm(r) / np.linalg.norm(b[live]) <= 1e-8
     for R in ranks:
         B.geom_destroy(R.g)

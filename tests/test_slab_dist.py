@@ -35,10 +35,18 @@ for t in range(T):
     U[t * ns:(t + 1) * ns] = float(t0 + t)
 halo_lo, halo_hi = slab.gauge_halo_exchange(U, L, xch)
 s = xch.allreduce_sum(torch.tensor([float(rank + 1)], dtype=torch.float64))
+# a lattice with open time boundaries: the chain is not closed
+xo = slab.FaceExchange(periodic=False)
+olo, ohi = torch.full_like(send_lo, -1.0), torch.full_like(send_lo, -1.0)
+xo(send_lo, send_hi, olo, ohi)
+oh_lo, oh_hi = slab.gauge_halo_exchange(U, L, xo)
 open(os.path.join(%r, "rank%%d.json" %% rank), "w").write(json.dumps({"rank": rank, "world": world, "t0": t0, "T": T, "below": xch.below, "above": xch.above,
                   "recv_lo": sorted(set(recv_lo.tolist())), "recv_hi": sorted(set(recv_hi.tolist())),
                   "halo_lo": sorted(set(halo_lo.real.flatten().tolist())),
-                  "halo_hi": sorted(set(halo_hi.real.flatten().tolist())), "sum": s.item()}))
+                  "halo_hi": sorted(set(halo_hi.real.flatten().tolist())), "sum": s.item(),
+                  "open_nbr": [xo.below, xo.above], "open_lo": sorted(set(olo.tolist())), "open_hi": sorted(set(ohi.tolist())),
+                  "open_halo": [None if h is None else sorted(set(h.real.flatten().tolist())) for h in (oh_lo, oh_hi)],
+                  "edges": slab.slab_edges(world, rank, 1)}))
 dist.barrier()
 dist.destroy_process_group()
 '''
@@ -68,6 +76,13 @@ def test_face_exchange_on_the_time_ring(tmp_path, world, port):
         assert d["halo_lo"] == [float((4 * r - 1) % L4)]
         assert d["halo_hi"] == [float((4 * r + 4) % L4)]
         assert d["sum"] == world * (world + 1) / 2
+        # open lattice: first rank has nobody below, last nobody above; those receive buffers stay untouched
+        first, last = r == 0, r == world - 1
+        assert d["open_nbr"] == [None if first else below, None if last else above]
+        assert d["open_lo"] == ([-1.0] if first else [100.0 * below + 2])
+        assert d["open_hi"] == ([-1.0] if last else [100.0 * above + 1])
+        assert d["open_halo"] == [None if first else [float(4 * r - 1)], None if last else [float(4 * r + 4)]]
+        assert d["edges"] == (1 if first else 0) | (2 if last else 0)
 
 
 def test_slab_bookkeeping():
