@@ -296,9 +296,9 @@ def run_ours(args):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the stencil kernel from the committed ncu --set full
-# capture (profiles/r01_v2_dw_pipe_kernel_f64_full.txt); keyed by (lattice, prec, recon).  None = not captured for
+# capture (profiles/r01_v3_dw_pipe_kernel_f64_full.txt); keyed by (lattice, prec, recon).  None = not captured for
 # that configuration.
-NCU_TRAFFIC = {("48x48x48x96", "f64", 18): 16878387000 + 2025411000}
+NCU_TRAFFIC = {("48x48x48x96", "f64", 18): 17142972000 + 2026305000}
 
 
 def run_e2e(torch, B, S, args, L, prec, recon, dist):
