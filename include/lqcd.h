@@ -71,7 +71,10 @@ typedef struct {
                        /* upper time face is an OPEN boundary of the lattice (first / last rank of a lattice with  */
                        /* open BC): that slice is frozen (D7) and nothing is exchanged through it.  0 = periodic.  */
 } lqcd_geom_desc;
-enum { LQCD_SLAB_OPEN_LO = 1, LQCD_SLAB_OPEN_HI = 2 };
+enum { LQCD_SLAB_OPEN_LO = 1, LQCD_SLAB_OPEN_HI = 2,
+       LQCD_SLAB_SF_HI = 4 };   /* the upper face is the SF boundary x4 = T (last rank of an SF lattice; its first rank */
+                                /* sets LQCD_SLAB_OPEN_LO: the frozen slice x4 = 0): no slice of the slab is frozen   */
+                                /* there, nothing is exchanged, and Csw! takes the boundary field W' from phiT      */
 
 /* Dirac parameters: kappa = 1/(2(m0+4)); csw; ct = c~_t (paper's cF), 1 = absent; mu = twisted
  * mass: D = A + 2 i kappa mu gamma5 - kappa H, D^+ = gamma5 D(-mu) gamma5; 0 = absent.
@@ -175,7 +178,8 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
  * Step 3 + 4 equal the whole-lattice operator restricted to the slab (rounding order of the last additions aside).
  * A lattice with OPEN time boundaries is decomposed the same way: its first / last rank set slab_edges; their outer
  * slice is frozen as in LQCD_BC_OPEN, the pack / face kernels leave that face alone and the ring is not closed
- * (theta[3] plays no role across an open boundary).  SF lattices are not decomposed.
+ * (theta[3] plays no role across an open boundary).  An SF lattice: first rank LQCD_SLAB_OPEN_LO, last rank
+ * LQCD_SLAB_SF_HI (with phiT in its geometry descriptor).
  * lqcd_clover_build_slab: Csw! on the slab; halo_lo / halo_hi = the time slice just below / above the slab, DEVICE,
  * canonical fp64 layout [L0 L1 L2][4][3][3] (a one-off exchange per configuration).  On a SLAB geometry the solver,
  * the even-odd operator and lqcd_clover_build return LQCD_EUNSUPPORTED (they would ignore the faces). */

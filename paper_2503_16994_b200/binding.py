@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(HERE, "liblqcd_b200.so")
 OK, EINVAL, ENOMEM, ECUDA, ENOTCONV, EBREAKDOWN, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB, BC_SLAB = 0, 1, 2, 3, 4
 F64, F32 = 0, 1
-SLAB_OPEN_LO, SLAB_OPEN_HI = 1, 2
+SLAB_OPEN_LO, SLAB_OPEN_HI, SLAB_SF_HI = 1, 2, 4
 RECON_18, RECON_12 = 18, 12
 FIELD_GAUGE, FIELD_SPINOR, FIELD_CLOVER, FIELD_WORKSPACE, FIELD_FACE = 0, 1, 2, 3, 4
 

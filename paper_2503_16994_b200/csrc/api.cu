@@ -195,7 +195,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   REQUIRE(desc && out, "lqcd_geom_create: NULL argument");
   *out = nullptr;
   REQUIRE(desc->bc >= LQCD_BC_PERIODIC && desc->bc <= LQCD_BC_SLAB, "lqcd_geom_create: bad bc %d", (int)desc->bc);
-  REQUIRE(desc->slab_edges >= 0 && desc->slab_edges <= 3 && (desc->bc == LQCD_BC_SLAB || desc->slab_edges == 0),
+  REQUIRE(desc->slab_edges >= 0 && desc->slab_edges <= 5 && (desc->bc == LQCD_BC_SLAB || desc->slab_edges == 0),
           "lqcd_geom_create: bad slab_edges %d", desc->slab_edges);
   for (int i = 0; i < 4; i++)
     REQUIRE(desc->L[i] >= 2 && desc->L[i] % 2 == 0, "lqcd_geom_create: extent L[%d]=%d must be even and >= 2 (R13)", i, desc->L[i]);
@@ -213,7 +213,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   Geom& g = h->g;
   for (int i = 0; i < 4; i++) g.L[i] = desc->L[i];
   g.bc = (int)desc->bc;
-  g.edges = desc->bc == LQCD_BC_SLAB ? (desc->slab_edges & 3) : 0;
+  g.edges = desc->bc == LQCD_BC_SLAB ? (desc->slab_edges & 7) : 0;
   g.Vh = (long long)g.L[0] * g.L[1] * g.L[2] * g.L[3] / 2;
   choose_tiling(g);
   h->has_theta = false;
@@ -354,13 +354,13 @@ lqcd_status lqcd_clover_build_slab(const lqcd_geom* h, const lqcd_dirac* d, cons
                                    lqcd_prec out_prec, void* stream) {
   REQUIRE(h && d && U64 && clover, "lqcd_clover_build_slab: NULL argument");
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_clover_build_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
-  REQUIRE((halo_lo || (h->g.edges & LQCD_SLAB_OPEN_LO)) && (halo_hi || (h->g.edges & LQCD_SLAB_OPEN_HI)),
+  REQUIRE((halo_lo || (h->g.edges & LQCD_SLAB_OPEN_LO)) && (halo_hi || (h->g.edges & (LQCD_SLAB_OPEN_HI | LQCD_SLAB_SF_HI))),
           "lqcd_clover_build_slab: a gauge halo is required on every face that is not an open boundary");
   REQUIRE(valid_prec(out_prec) && valid_recon(recon), "lqcd_clover_build_slab: bad precision / recon");
   REQUIRE(clover != U64 && clover_inv != U64 && clover != clover_inv, "lqcd_clover_build_slab: aliased buffers");
   CloverParm cp;
   cp.kappa = d->kappa; cp.csw = d->csw; cp.ct = d->ct;
-  for (int i = 0; i < 3; i++) cp.phiT[i] = 0.0;
+  for (int i = 0; i < 3; i++) cp.phiT[i] = h->desc.phiT[i];
   CUDA_TRY(clover_build(h->g, cp, U64, (int)recon, clover, clover_inv, (int)out_prec, as_stream(stream), halo_lo, halo_hi),
            "clover_build (slab)");
   return LQCD_OK;

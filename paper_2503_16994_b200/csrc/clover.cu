@@ -69,7 +69,7 @@ __device__ __forceinline__ m3 link_at(const CloverCtx& c, const SitePos& sp, int
   const Geom& g = c.g;
   constexpr int NCU = RECON == 12 ? 6 : 9;
   m3 r;
-  const bool sf = (g.bc == LQCD_BC_SF_ORBI || g.bc == LQCD_BC_SF_AFWB);
+  const bool sf = (g.bc == LQCD_BC_SF_ORBI || g.bc == LQCD_BC_SF_AFWB) || (g.bc == LQCD_BC_SLAB && (g.edges & LQCD_SLAB_SF_HI));
   const int x3 = sp.x3 + (mu == 3 ? dm : 0) + (nu == 3 ? dn : 0);
   if (sf && x3 == g.L[3]) {   // diagonal: its own transpose; dagger = conjugate
 #pragma unroll
@@ -264,9 +264,9 @@ __global__ void __launch_bounds__(CLV_THREADS, CLV_MINB) clover_kernel(const Clo
   double dadd = 0.0;
   if (!fz && g.bc != LQCD_BC_PERIODIC && cp.ct != 1.0) {  // R10: + 2 kappa (ct - 1) next to the frozen slices
     const bool slab = g.bc == LQCD_BC_SLAB;   // a slab has the term only next to its open faces
-    const int last = (g.bc == LQCD_BC_OPEN || slab) ? g.L[3] - 2 : g.L[3] - 1;
+    const int last = (g.bc == LQCD_BC_OPEN || (slab && (g.edges & LQCD_SLAB_OPEN_HI))) ? g.L[3] - 2 : g.L[3] - 1;
     if (x3 == 1 && (!slab || (g.edges & LQCD_SLAB_OPEN_LO))) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
-    if (x3 == last && (!slab || (g.edges & LQCD_SLAB_OPEN_HI))) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
+    if (x3 == last && (!slab || (g.edges & (LQCD_SLAB_OPEN_HI | LQCD_SLAB_SF_HI)))) dadd += 2.0 * cp.kappa * (cp.ct - 1.0);
   }
   const size_t TV = g.TV;
 #pragma unroll 1

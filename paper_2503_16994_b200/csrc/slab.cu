@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(128) slab_pack_kernel(const Geom g, const Slab
   const int id = blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= 2 * a.ns) return;
   const bool upper = id >= a.ns;   // upper face: slice L3-1 -> send_hi
-  if (g.edges & (upper ? LQCD_SLAB_OPEN_HI : LQCD_SLAB_OPEN_LO)) return;   // open boundary: nothing crosses it
+  if (g.edges & (upper ? (LQCD_SLAB_OPEN_HI | LQCD_SLAB_SF_HI) : LQCD_SLAB_OPEN_LO)) return;   // open / SF boundary: nothing crosses it
   const int n = upper ? id - a.ns : id;
   int x[4], p, tile, j;
   spatial_site(g, n, upper ? g.L[3] - 1 : 0, x);
@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(128) slab_faces_kernel(const Geom g, const Sla
   const int id = blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= 2 * a.ns) return;
   const bool upper = id >= a.ns;   // upper face: forward hop of slice L3-1 from recv_hi
-  if (g.edges & (upper ? LQCD_SLAB_OPEN_HI : LQCD_SLAB_OPEN_LO)) return;   // open boundary: frozen slice, no hop
+  if (g.edges & (upper ? (LQCD_SLAB_OPEN_HI | LQCD_SLAB_SF_HI) : LQCD_SLAB_OPEN_LO)) return;   // open / SF boundary: no hop
   const int n = upper ? id - a.ns : id;
   int x[4], p, tile, j;
   spatial_site(g, n, upper ? g.L[3] - 1 : 0, x);

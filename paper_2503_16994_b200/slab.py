@@ -47,16 +47,18 @@ def slab_edges(world, rank, bc=B.BC_PERIODIC):
     """lqcd_geom_desc.slab_edges of this rank: which of its faces are open boundaries of the lattice."""
     if bc == B.BC_PERIODIC:
         return 0
-    if bc != B.BC_OPEN:
-        raise ValueError("only lattices periodic or open in time are decomposed (bc=%r)" % (bc,))
-    return (B.SLAB_OPEN_LO if rank == 0 else 0) | (B.SLAB_OPEN_HI if rank == world - 1 else 0)
+    if bc not in (B.BC_OPEN, B.BC_SF_ORBI, B.BC_SF_AFWB):
+        raise ValueError("bad time boundary condition %r" % (bc,))
+    top = B.SLAB_OPEN_HI if bc == B.BC_OPEN else B.SLAB_SF_HI   # SF: no frozen slice at the top, boundary field W'
+    return (B.SLAB_OPEN_LO if rank == 0 else 0) | (top if rank == world - 1 else 0)
 
 
-def slab_geom_create(L, world, theta=None, device=0, rank=0, bc=B.BC_PERIODIC):
-    """Geometry handle of one rank's slab of the lattice L (bc: periodic in time -- antiperiodic = theta4 = pi -- or
-    open, in which case the first and last rank get a frozen outer slice)."""
+def slab_geom_create(L, world, theta=None, device=0, rank=0, bc=B.BC_PERIODIC, phiT=None):
+    """Geometry handle of one rank's slab of the lattice L (bc: periodic in time -- antiperiodic = theta4 = pi --,
+    open: the first and last rank get a frozen outer slice, or SF: frozen slice x4 = 0 on the first rank, boundary
+    field W' = exp(i phiT / L_k) above the last rank's top slice)."""
     T = slab_extent(L[3], world)
-    return B.geom_create((L[0], L[1], L[2], T), B.BC_SLAB, slab_theta(theta, L[3], world), device=device,
+    return B.geom_create((L[0], L[1], L[2], T), B.BC_SLAB, slab_theta(theta, L[3], world), phiT=phiT, device=device,
                          slab_edges=slab_edges(world, rank, bc))
 
 

@@ -29,11 +29,11 @@ def mode(request):
 class Rank:
     """What one rank of the decomposition holds."""
 
-    def __init__(self, L, P, r, theta, U, kappa, csw, prec, recon, bc=B.BC_PERIODIC, ct=1.0):
+    def __init__(self, L, P, r, theta, U, kappa, csw, prec, recon, bc=B.BC_PERIODIC, ct=1.0, phiT=None):
         self.T = slab.slab_extent(L[3], P)
         self.ns = L[0] * L[1] * L[2]
         self.lo, self.hi = r * self.T * self.ns, (r + 1) * self.T * self.ns   # canonical site range (time slowest)
-        self.g = slab.slab_geom_create(L, P, theta, rank=r, bc=bc)
+        self.g = slab.slab_geom_create(L, P, theta, rank=r, bc=bc, phiT=phiT)
         self.nbr = slab.ring_neighbours(P, r, bc == B.BC_PERIODIC)
         Uc = to_dev(U[self.lo:self.hi])
         self.U64 = B.alloc_field(self.g, B.FIELD_GAUGE, B.F64, recon)
@@ -130,6 +130,34 @@ def test_slab_dw_open_boundaries(mode, L, P, prec):
         assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
     for dagger in (False, True):
         ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=B.BC_OPEN, theta=theta, dagger=dagger)
+        got = slab_dw(ranks, kappa, psi, prec, recon, dagger)
+        assert site_rel_err(got, ref, mask) <= TOL[prec]
+        assert np.all(got[~mask] == 0)
+    for R in ranks:
+        B.geom_destroy(R.g)
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
+@pytest.mark.parametrize("L,P", [((4, 4, 4, 8), 2), ((4, 8, 4, 12), 3), ((4, 4, 4, 8), 1)])
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_slab_dw_sf_boundaries(mode, L, P, prec):
+    """Schroedinger-functional lattice in slabs: frozen slice x4 = 0 on the first rank, boundary field W' (phiT) above
+    the last rank's top slice in the clover term, c~_t on both ends.  Against the oracle's SF operator."""
+    kappa, csw, ct, theta, recon, bc = 0.1355, 1.8, 1.1, (0.5, 0.5, 0.5, 0.0), B.RECON_18, B.BC_SF_ORBI
+    U = synth.apply_sf_boundary(L, synth.smooth_gauge(L, 131))
+    psi = synth.gaussian_spinor(L, 132)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc, phiT=synth.SF_PHIT, ct=ct)
+    Uo, psio, Ao = (round_f32(U), round_f32(psi), round_f32(A)) if prec == B.F32 else (U, psi, A)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, prec, recon, bc=bc, ct=ct, phiT=synth.SF_PHIT) for r in range(P)]
+    t = np.arange(psi.shape[0]) // (L[0] * L[1] * L[2])
+    mask = t >= 1
+    for R in ranks:
+        got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
+        B.clover_export(R.g, R.A, got, prec)
+        torch.cuda.synchronize()
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+    for dagger in (False, True):
+        ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=bc, theta=theta, dagger=dagger)
         got = slab_dw(ranks, kappa, psi, prec, recon, dagger)
         assert site_rel_err(got, ref, mask) <= TOL[prec]
         assert np.all(got[~mask] == 0)
