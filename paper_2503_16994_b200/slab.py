@@ -208,3 +208,38 @@ class SlabCommunicator:
 def cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, communicator, **kw):
     """D x = b on the decomposed lattice; every rank calls this with its slab.  Returns lqcd_cg_solve's info dict."""
     return B.cg_solve_slab(g, kappa, U64, clover64, b, x, workspace, communicator.struct, **kw)
+
+
+def propagator_slab(g, L, world, rank, kappa, U64, clover64, y, columns, workspace, communicator, **kw):
+    """propagator! point-source method on the decomposed lattice: for column = 3*spin + colour solve
+    D x = delta_y e_column with lqcd_cg_solve_slab.  y: source position on the WHOLE lattice (only the rank whose slab
+    holds y[3] has a non-zero source); columns: 12 consecutive internal fp64 spinor fields of this rank's slab.
+    Returns the 12 info dicts."""
+    T = slab_extent(L[3], world)
+    t0 = slab_origin(L[3], world, rank)
+    mine = t0 <= int(y[3]) < t0 + T
+    fb = B.field_bytes(g, B.FIELD_SPINOR, B.F64)
+    src = B.alloc_field(g, B.FIELD_SPINOR, B.F64)
+    infos = []
+    for col in range(12):
+        if mine:
+            B.point_source(g, (y[0], y[1], y[2], int(y[3]) - t0), col // 3, col % 3, src)
+        else:
+            src.zero_()
+        infos.append(B.cg_solve_slab(g, kappa, U64, clover64, src, columns[col * fb:(col + 1) * fb], workspace,
+                                     communicator.struct, **kw))
+    return infos
+
+
+def correlator_ps_slab(g, L, world, rank, columns, ncol, workspace, communicator, prec=B.F64):
+    """C(x4) for all x4 of the whole lattice on every rank: each rank reduces its own time slices
+    (lqcd_correlator_ps), the slices are put in place in a zero vector of length L4 and summed over the ranks."""
+    import torch
+
+    T = slab_extent(L[3], world)
+    t0 = slab_origin(L[3], world, rank)
+    local = B.correlator_ps(g, columns, ncol, workspace, T, prec)
+    C = torch.zeros(int(L[3]), dtype=torch.float64, device=columns.device)
+    C[t0:t0 + T] = torch.tensor(list(local), dtype=torch.float64, device=columns.device)
+    communicator.exchange.allreduce_sum(C)
+    return C.cpu().tolist()

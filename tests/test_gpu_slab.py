@@ -332,3 +332,58 @@ def test_cg_over_slabs(L, P, theta, bc, mixed):
     assert np.linalg.norm(r) / np.linalg.norm(b[live]) <= 1e-8
     for R in ranks:
         B.geom_destroy(R.g)
+
+
+@pytest.mark.timeout(600)
+def test_propagator_and_correlator_over_slabs():
+    """The paper's end product on a decomposed lattice: 12 point-source columns by
+    lqcd_cg_solve_slab on two slabs (threads as ranks), then C(x4) assembled from the slabs' own time slices, against
+    the oracle's CG + correlator on the whole lattice.  The source sits in the second slab."""
+    import threading
+
+    L, P, kappa, csw, theta, y = (4, 4, 4, 8), 2, 0.125, 1.0, (0, 0, 0, np.pi), (1, 2, 3, 5)
+    U = synth.smooth_gauge(L, 141)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    ranks = [Rank(L, P, r, theta, U, kappa, csw, B.F64, B.RECON_18) for r in range(P)]
+    ring = ThreadRing(P)
+    V = synth.vol(L)
+    got_cols = np.empty((12, V, 4, 3), dtype=np.complex128)
+    corr, errors = [None] * P, []
+
+    def run(r):
+        try:
+            R = ranks[r]
+            comm = slab.SlabCommunicator(R.g, ring.view(r))
+            ws = B.alloc_field(R.g, B.FIELD_WORKSPACE)
+            fb = B.field_bytes(R.g, B.FIELD_SPINOR)
+            cols = torch.empty(12 * fb, dtype=torch.uint8, device="cuda")
+            infos = slab.propagator_slab(R.g, L, P, r, kappa, R.U, R.A, y, cols, ws, comm, tol=1e-12, maxiter=4000)
+            assert all(i["status"] == B.OK for i in infos)
+            corr[r] = slab.correlator_ps_slab(R.g, L, P, r, cols, 12, ws, comm)
+            o = torch.empty((R.hi - R.lo, 4, 3), dtype=torch.complex128, device="cuda")
+            for c in range(12):
+                B.spinor_export(R.g, cols[c * fb:(c + 1) * fb], o)
+                torch.cuda.synchronize()
+                got_cols[c, R.lo:R.hi] = o.cpu().numpy()
+        except Exception as e:   # noqa: BLE001
+            errors.append(e)
+            ring.barrier.abort()
+
+    threads = [threading.Thread(target=run, args=(r,)) for r in range(P)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(500)
+    assert not errors, errors
+    ref_cols = []
+    for c in range(12):
+        b = synth.point_source(L, y, c // 3, c % 3)
+        ref_cols.append(oracle.cg(L, U, b, kappa, A, theta=theta, tol=1e-12)[0])
+    ref_cols = np.array(ref_cols)
+    assert np.linalg.norm(got_cols - ref_cols) / np.linalg.norm(ref_cols) <= 1e-8
+    ref = oracle.correlator_ps(L, ref_cols)
+    for r in range(P):
+        assert np.max(np.abs(np.array(corr[r]) - ref) / ref) <= 1e-8
+    assert int(np.argmax(ref)) == y[3]
+    for R in ranks:
+        B.geom_destroy(R.g)
