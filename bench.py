@@ -454,6 +454,7 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
     rows.update(run_config2(torch, B, synth, peak))
     rows.update(run_config3(torch, B, synth, peak))
     rows.update(run_config4(torch, B, synth, peak))
+    rows.update(run_config5b(torch, B, synth, peak))
     return rows
 
 
@@ -477,6 +478,42 @@ def run_config2(torch, B, synth, peak):
     del S, U32
     torch.cuda.empty_cache()
     return out
+
+
+def run_config5b(torch, B, synth, peak):
+    """configs[4], second lattice: 64^3 x 128 periodic, kappa = 0.137, csw = 1.9: Dw in fp64 / fp32 with 18- and 12-real
+    links as a fraction of the HBM roofline (51.5 / 25.8 GB compulsory per application: the largest single-GPU case)."""
+    L, kappa, csw = (64, 64, 64, 128), 0.137, 1.9
+    free, _ = torch.cuda.mem_get_info()
+    if free < 130 * (1 << 30):
+        return {"a4_dw_64x64x64x128": {"skipped": "needs ~110 GB of free device memory, %d GB free" % (free >> 30)}}
+    S = Setup(torch, B, synth, L, B.BC_PERIODIC, None, None, kappa, csw, 5, 0, [B.F64, B.F32], [18])
+    g, V = S.g, S.V
+    out = {"lattice": "64x64x64x128", "clover_build_ms": round(S.clover_ms, 3)}
+    for r in (18, 12):
+        if r == 12:
+            canon = torch.empty((V, 4, 3, 3), dtype=torch.complex128, device="cuda")
+            B.gauge_export(g, S.U[(B.F64, 18)], canon, B.F64, 18)
+            S.U[(B.F64, 12)] = B.alloc_field(g, B.FIELD_GAUGE, B.F64, 12)
+            B.gauge_import(g, canon, S.U[(B.F64, 12)], B.F64, 12)
+            del canon
+            del S.U[(B.F64, 18)], S.U[(B.F32, 18)]
+            torch.cuda.empty_cache()
+        if (B.F32, r) not in S.U:
+            S.U[(B.F32, r)] = B.alloc_field(g, B.FIELD_GAUGE, B.F32, r)
+            B.field_to_f32(g, B.FIELD_GAUGE, r, S.U[(B.F64, r)], S.U[(B.F32, r)])
+        for p, pname, rb in ((B.F64, "f64", 8), (B.F32, "f32", 4)):
+            for dag, fn in (("dw", B.dw_apply), ("dwdag", B.dwdag_apply)):
+                ms = time_calls(torch, lambda: fn(g, kappa, S.U[(p, r)], S.A[p], S.psi[p], S.out[p], p, r), 5, 2)
+                gb = REALS_DW[r] * rb * V / (ms * 1e-3) / 1e9
+                out["%s_%s_recon%d" % (dag, pname, r)] = {
+                    "ms": round(ms, 4), "GFLOP/s": round(FLOP_DW * V / ms / 1e6, 1), "GB/s": round(gb, 1),
+                    "frac_measured_peak": round(gb / peak, 4)}
+    out["kernel"] = B.dw_plan(g, B.F64, 18, True)
+    S.close()
+    del S
+    torch.cuda.empty_cache()
+    return {"a4_dw_64x64x64x128": out}
 
 
 def run_config3(torch, B, synth, peak):
