@@ -905,7 +905,14 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
   const size_t V = (size_t)2 * h->g.Vh;
   const size_t gc = V * 36 * sizeof(double2), sc = V * 12 * sizeof(double2);
   void *dUc = nullptr, *dSc = nullptr, *dU64 = nullptr, *dU = nullptr, *dA = nullptr, *dIn = nullptr, *dOut = nullptr;
+  cudaStream_t s1 = nullptr, s2 = nullptr;
+  cudaEvent_t ev_u = nullptr, ev_s = nullptr;
   auto cleanup = [&]() {
+    cudaDeviceSynchronize();
+    if (ev_u) cudaEventDestroy(ev_u);
+    if (ev_s) cudaEventDestroy(ev_s);
+    if (s1) cudaStreamDestroy(s1);
+    if (s2) cudaStreamDestroy(s2);
     cudaFree(dUc); cudaFree(dSc); cudaFree(dU64); if (dU != dU64) cudaFree(dU); cudaFree(dA); cudaFree(dIn); cudaFree(dOut);
     lqcd_geom_destroy(h);
   };
@@ -916,22 +923,33 @@ lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, 
   HTRY(cudaMalloc(&dU64, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F64, recon)), "cudaMalloc");
   HTRY(cudaMalloc(&dIn, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
   HTRY(cudaMalloc(&dOut, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
-  HTRY(cudaMemcpy(dUc, U_canon_host, gc, cudaMemcpyHostToDevice), "H2D gauge");
-  HTRY(cudaMemcpy(dSc, in_canon_host, sc, cudaMemcpyHostToDevice), "H2D spinor");
-  LTRY(lqcd_gauge_import(h, dUc, dU64, LQCD_F64, recon, nullptr));
+  // two streams: the spinor's H2D copy (s2) runs while the gauge field is imported and the clover term built (s1);
+  // with pinned host buffers the copies are truly asynchronous, with pageable ones they are staged but still ordered
+  HTRY(cudaStreamCreate(&s1), "cudaStreamCreate");
+  HTRY(cudaStreamCreate(&s2), "cudaStreamCreate");
+  HTRY(cudaEventCreateWithFlags(&ev_u, cudaEventDisableTiming), "cudaEventCreate");
+  HTRY(cudaEventCreateWithFlags(&ev_s, cudaEventDisableTiming), "cudaEventCreate");
+  HTRY(cudaMemcpyAsync(dUc, U_canon_host, gc, cudaMemcpyHostToDevice, s1), "H2D gauge");
+  HTRY(cudaEventRecord(ev_u, s1), "event");
+  HTRY(cudaStreamWaitEvent(s2, ev_u, 0), "wait");   // same PCIe direction: the spinor follows the gauge field
+  HTRY(cudaMemcpyAsync(dSc, in_canon_host, sc, cudaMemcpyHostToDevice, s2), "H2D spinor");
+  LTRY(lqcd_spinor_import(h, dSc, dIn, prec, s2));
+  HTRY(cudaEventRecord(ev_s, s2), "event");
+  LTRY(lqcd_gauge_import(h, dUc, dU64, LQCD_F64, recon, s1));
   if (d->csw != 0.0 || (desc->bc != LQCD_BC_PERIODIC && d->ct != 1.0)) {
     HTRY(cudaMalloc(&dA, lqcd_field_bytes(h, LQCD_FIELD_CLOVER, prec, recon)), "cudaMalloc");
-    LTRY(lqcd_clover_build(h, d, dU64, recon, dA, nullptr, prec, nullptr));
+    LTRY(lqcd_clover_build(h, d, dU64, recon, dA, nullptr, prec, s1));
   }
   if (prec == LQCD_F64) dU = dU64;
   else {
     HTRY(cudaMalloc(&dU, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F32, recon)), "cudaMalloc");
-    LTRY(lqcd_gauge_import(h, dUc, dU, LQCD_F32, recon, nullptr));
+    LTRY(lqcd_gauge_import(h, dUc, dU, LQCD_F32, recon, s1));
   }
-  LTRY(lqcd_spinor_import(h, dSc, dIn, prec, nullptr));
-  LTRY(dw_common(h, d, dU, dA, dIn, dOut, prec, recon, nullptr, dagger != 0));
-  LTRY(lqcd_spinor_export(h, dOut, dSc, prec, nullptr));
-  HTRY(cudaMemcpy(out_canon_host, dSc, sc, cudaMemcpyDeviceToHost), "D2H spinor");
+  HTRY(cudaStreamWaitEvent(s1, ev_s, 0), "wait");
+  LTRY(dw_common(h, d, dU, dA, dIn, dOut, prec, recon, s1, dagger != 0));
+  LTRY(lqcd_spinor_export(h, dOut, dSc, prec, s1));
+  HTRY(cudaMemcpyAsync(out_canon_host, dSc, sc, cudaMemcpyDeviceToHost, s1), "D2H spinor");
+  HTRY(cudaStreamSynchronize(s1), "sync");
   cleanup();
 #undef HTRY
 #undef LTRY
