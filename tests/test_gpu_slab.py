@@ -96,7 +96,7 @@ def test_slab_dw_equals_whole_lattice(mode, L, P, theta, prec, recon):
         got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
         B.clover_export(R.g, R.A, got, prec)
         torch.cuda.synchronize()
-        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 2.4e-7)  # fp32 storage: the fp64 build rounded once; one ulp of slack at |A| < 2
     for dagger in (False, True):
         ref = oracle.dw(L, Uo, psio, kappa, Ao, theta=theta, dagger=dagger)
         assert site_rel_err(slab_dw(ranks, kappa, psi, prec, recon, dagger), ref) <= TOL[prec]
@@ -127,7 +127,7 @@ def test_slab_dw_open_boundaries(mode, L, P, prec):
         got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
         B.clover_export(R.g, R.A, got, prec)
         torch.cuda.synchronize()
-        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 2.4e-7)  # fp32 storage: the fp64 build rounded once; one ulp of slack at |A| < 2
     for dagger in (False, True):
         ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=B.BC_OPEN, theta=theta, dagger=dagger)
         got = slab_dw(ranks, kappa, psi, prec, recon, dagger)
@@ -155,7 +155,7 @@ def test_slab_dw_sf_boundaries(mode, L, P, prec):
         got = torch.empty((R.hi - R.lo, 2, 6, 6), dtype=torch.complex128, device="cuda")
         B.clover_export(R.g, R.A, got, prec)
         torch.cuda.synchronize()
-        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 0.0)
+        assert np.max(np.abs(got.cpu().numpy() - Ao[R.lo:R.hi])) <= (2e-14 if prec == B.F64 else 2.4e-7)  # fp32 storage: the fp64 build rounded once; one ulp of slack at |A| < 2
     for dagger in (False, True):
         ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=bc, theta=theta, dagger=dagger)
         got = slab_dw(ranks, kappa, psi, prec, recon, dagger)
