@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-rows", action="store_true", help="skip the per-row extras (rank 0, N=1)")
+    ap.add_argument("--decompose", action="store_true",
+                    help="NEXT-3 (opt-in, not the driver's mode): ONE lattice cut into --gpus time slabs, half-spinor "
+                         "faces exchanged between ring neighbours (NCCL); strong scaling")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--kappa", type=float, default=0.137)
@@ -628,6 +631,103 @@ def cpu_baseline(np, torch, S, args):
                       "recipe (kappa=%g csw=%g), %.1f s" % (steps, "x".join(map(str, L)), args.kappa, args.csw, dt)}
 
 
+def run_decomposed(args):
+    """--decompose: the lattice of --lattice as WORLD_SIZE time slabs, one per GPU.
+    A step = D then D^+ on the whole lattice: per rank pack -> face exchange (side stream) || slab stencil -> faces.
+    Every rank draws its own slab of links (any stack of SU(3) slabs is a valid gauge field); the clover term sees the
+    neighbours' slices through the real gauge-halo exchange.  Only the N = 1 case (the slab exchanging with itself)
+    has been run: the boxes of this build have one GPU."""
+    import torch
+
+    from paper_2503_16994_b200 import binding as B
+    from paper_2503_16994_b200 import slab, synth
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU fallback")
+    B.lib()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    L = tuple(int(v) for v in args.lattice.lower().split("x"))
+    prec = B.F64 if args.prec == "f64" else B.F32
+    recon, rb = args.recon, (8 if args.prec == "f64" else 4)
+    T = slab.slab_extent(L[3], world)
+    Ls = (L[0], L[1], L[2], T)
+    dev = torch.device("cuda", local)
+    g = slab.slab_geom_create(L, world, None, device=local, rank=rank)
+    Uc = synth.smooth_gauge_torch(Ls, synth.seed_for(5, 0) + 100 * rank, dev)
+    xch = slab.FaceExchange()
+    halo_lo, halo_hi = slab.gauge_halo_exchange(Uc, L, xch)
+    U64 = B.alloc_field(g, B.FIELD_GAUGE, B.F64, recon)
+    B.gauge_import(g, Uc, U64, B.F64, recon)
+    A = B.alloc_field(g, B.FIELD_CLOVER, prec)
+    B.clover_build_slab(g, args.kappa, args.csw, U64, halo_lo, halo_hi, A, None, recon, prec)
+    U = U64
+    if prec == B.F32:
+        U = B.alloc_field(g, B.FIELD_GAUGE, B.F32, recon)
+        B.field_to_f32(g, B.FIELD_GAUGE, recon, U64, U)
+    psi, out, out2 = (B.alloc_field(g, B.FIELD_SPINOR, prec) for _ in range(3))
+    B.spinor_import(g, synth.gaussian_spinor_torch(Ls, synth.seed_for(5, 1) + 100 * rank, dev), psi, prec)
+    del Uc, halo_lo, halo_hi
+    D = slab.SlabDirac(g, args.kappa, U, A, prec, recon, exchange=xch)
+
+    def step():
+        D.apply(psi, out, False)
+        D.apply(out, out2, True)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.05)
+    l0 = B.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    launches = B.launch_count() - l0
+    ms_local = e0.elapsed_time(e1)
+    clocks = sampler.result()
+    if dist is not None:
+        dist.barrier()
+    ms = max_over_ranks(torch, dist, ms_local, "cuda") / args.steps
+    Vs = synth.vol(Ls)
+    peak, peak_src = measured_peaks()
+    achieved = 2 * REALS_DW[recon] * rb * Vs / (ms_local / args.steps * 1e-3) / 1e9   # this rank's two stencil launches
+    face = B.field_bytes(g, B.FIELD_FACE, prec)
+    result = {
+        "metric": "Dw GFLOP/s (clover Wilson-Dirac, 1872 flop/site/application)",
+        "value": round(2.0 * FLOP_DW * synth.vol(L) / (ms * 1e-3) / 1e9, 1), "unit": "GFLOP/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms, 4), "higher_is_better": True,
+        "scaling": "strong", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
+        "config": {"workload": "Dw^+Dw application, %s periodic SU(3) as %d time slabs of %d slices, kappa=%g csw=%g, recon=%d"
+                               % (args.lattice, world, T, args.kappa, args.csw, recon),
+                   "step": "per rank: 2 x (lqcd_dw_slab_pack, face exchange, lqcd_dw_apply / lqcd_dwdag_apply, lqcd_dw_slab_faces)",
+                   "l2": "inputs larger than L2, no flush", "parallelism": "time slabs x%d, half-spinor faces over NCCL" % world,
+                   "face_bytes_per_application_per_rank": 2 * face},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": B.dw_plan(g, prec, recon, True).split("<")[0], "achieved": round(achieved, 1),
+                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4), "peak_source": peak_src,
+                     "note": "whole step of this rank (pack + stencil + faces) against the stencil's compulsory bytes",
+                     "traffic": None},
+        "e2e": None,
+    }
+    B.geom_destroy(g)
+    if rank == 0:
+        print(json.dumps(result))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def run_reference(args):
     """--impl reference: there is no reference code (PAPER.md only); the arm is the fp64 oracle on the host cores."""
     rank, world, _ = dist_env()
@@ -661,6 +761,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decompose:
+        run_decomposed(args)
     else:
         run_ours(args)
 
