@@ -1,8 +1,10 @@
 """Time-direction domain decomposition over torch.distributed.
 
-One process per GPU; rank r owns the time slab [r*T, (r+1)*T) of a lattice periodic in time (T = L4 / world).
+One process per GPU; rank r owns the time slab [r*T, (r+1)*T) of the lattice (T = L4 / world).  The lattice may be
+periodic in time (antiperiodic = theta4 = pi), open, or Schroedinger-functional: on an open / SF lattice the first
+and last rank carry the physical boundary (lqcd_geom_desc.slab_edges) and the chain of ranks is not closed.
 Every step of the arithmetic runs in the library's kernels (lqcd_dw_slab_pack, lqcd_dw_apply / lqcd_dwdag_apply on the
-LQCD_BC_SLAB geometry, lqcd_dw_slab_faces); this module only decides who owns what and moves the two half-spinor
+LQCD_BC_SLAB geometry, lqcd_dw_slab_faces, lqcd_clover_build_slab, lqcd_cg_solve_slab); this module only decides who owns what and moves the two half-spinor
 faces per application between ring neighbours (NCCL send/recv over NVLink on GPUs; gloo in the CPU tests of the
 exchange logic).  The exchange runs on its own stream and overlaps the interior stencil kernel.
 
