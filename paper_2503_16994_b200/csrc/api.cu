@@ -118,10 +118,15 @@ static cudaStream_t as_stream(void* s) { return (cudaStream_t)s; }
 
 static size_t spinor_complex(const Geom& g) { return (size_t)2 * g.Vh * 12; }
 static size_t elem_bytes(lqcd_prec p) { return p == LQCD_F64 ? sizeof(double2) : sizeof(float2); }
+// Length of the per-CTA partial-sum buffer: the largest grid any reducing kernel can have on this geometry --
+// 2 * ntiles (dw_mode = split: one CTA per tile parity), sm_count * 8 resident CTAs (persistent one-thread-per-site
+// kernels: at most 8 CTAs of >= 128 threads with > 64 registers fit an SM), two values per CTA of the BLAS-1 kernels
+// (dot: re and im; grid <= 8 CTAs per SM) -- plus 64 doubles of scratch at the end.
 static size_t partial_len(const Geom& g) {
-  size_t n = (size_t)g.ntiles;
-  size_t r = (size_t)2 * reduce_blocks(spinor_complex(g));
-  return (n > r ? n : r) + 64;
+  size_t n = (size_t)2 * g.ntiles;
+  const size_t r = (size_t)2 * 8 * (g.sm_count > 0 ? g.sm_count : 148);
+  if (r > n) n = r;
+  return n + 64;
 }
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -145,6 +150,21 @@ static const int WS_SPINORS32 = 6;
 }  // namespace lqcd
 
 using namespace lqcd;
+
+// Every entry point that takes a geometry runs on the device the geometry was created for (lqcd_geom_desc.device)
+// and leaves the caller's current device as it found it.
+namespace {
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  explicit DeviceGuard(const lqcd_geom* h) : DeviceGuard(h ? h->desc.device : 0) {}
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+bool good_kappa(const lqcd_dirac* d) { return d->kappa > 0.0 && d->kappa < 1e300; }
+}  // namespace
 
 #define REQUIRE(cond, ...)          \
   do {                              \
@@ -206,7 +226,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
     return LQCD_ECUDA;
   }
   REQUIRE(desc->device >= 0 && desc->device < ndev, "lqcd_geom_create: bad device %d", desc->device);
-  CUDA_TRY(cudaSetDevice(desc->device), "cudaSetDevice");
+  DeviceGuard dg(desc->device);
   lqcd_geom* h = (lqcd_geom*)calloc(1, sizeof(lqcd_geom));
   if (!h) { set_error("out of host memory"); return LQCD_ENOMEM; }
   h->desc = *desc;
@@ -229,6 +249,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
   h->smem_optin = (int)prop.sharedMemPerBlockOptin;
   g.sm_count = h->sm_count;
   g.smem_optin = h->smem_optin;
+  set_reduce_sm_count(h->sm_count);
   {  // neighbour-tile table (a1): 8 neighbours + time origin per tile
     std::vector<int> tab((size_t)g.ntiles * TILE_TAB, 0);
     for (int t = 0; t < g.ntiles; t++) {
@@ -257,6 +278,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
 
 lqcd_status lqcd_geom_destroy(lqcd_geom* g) {
   if (g) {
+    DeviceGuard dg(g);
     if (g->g.tile_tab) cudaFree((void*)g->g.tile_tab);
     free(g);
   }
@@ -295,6 +317,7 @@ size_t lqcd_field_bytes(const lqcd_geom* h, lqcd_field_kind kind, lqcd_prec prec
 
 lqcd_status lqcd_gauge_import(const lqcd_geom* h, const void* canon, void* U, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && canon && U && canon != U, "lqcd_gauge_import: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_gauge_import: bad precision / recon");
   CUDA_TRY(DISPATCH_PREC(prec, gauge_import<double>(h->g, canon, U, recon, as_stream(stream)),
                          gauge_import<float>(h->g, canon, U, recon, as_stream(stream))), "gauge_import");
@@ -302,6 +325,7 @@ lqcd_status lqcd_gauge_import(const lqcd_geom* h, const void* canon, void* U, lq
 }
 lqcd_status lqcd_gauge_export(const lqcd_geom* h, const void* U, void* canon, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && canon && U && canon != U, "lqcd_gauge_export: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_gauge_export: bad precision / recon");
   CUDA_TRY(DISPATCH_PREC(prec, gauge_export<double>(h->g, U, canon, recon, as_stream(stream)),
                          gauge_export<float>(h->g, U, canon, recon, as_stream(stream))), "gauge_export");
@@ -309,6 +333,7 @@ lqcd_status lqcd_gauge_export(const lqcd_geom* h, const void* U, void* canon, lq
 }
 lqcd_status lqcd_spinor_import(const lqcd_geom* h, const void* canon, void* psi, lqcd_prec prec, void* stream) {
   REQUIRE(h && canon && psi && canon != psi, "lqcd_spinor_import: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_spinor_import: bad precision");
   CUDA_TRY(DISPATCH_PREC(prec, spinor_import<double>(h->g, canon, psi, as_stream(stream)),
                          spinor_import<float>(h->g, canon, psi, as_stream(stream))), "spinor_import");
@@ -316,6 +341,7 @@ lqcd_status lqcd_spinor_import(const lqcd_geom* h, const void* canon, void* psi,
 }
 lqcd_status lqcd_spinor_export(const lqcd_geom* h, const void* psi, void* canon, lqcd_prec prec, void* stream) {
   REQUIRE(h && canon && psi && canon != psi, "lqcd_spinor_export: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_spinor_export: bad precision");
   CUDA_TRY(DISPATCH_PREC(prec, spinor_export<double>(h->g, psi, canon, as_stream(stream)),
                          spinor_export<float>(h->g, psi, canon, as_stream(stream))), "spinor_export");
@@ -323,6 +349,7 @@ lqcd_status lqcd_spinor_export(const lqcd_geom* h, const void* psi, void* canon,
 }
 lqcd_status lqcd_clover_export(const lqcd_geom* h, const void* clover, void* canon, lqcd_prec prec, void* stream) {
   REQUIRE(h && canon && clover && canon != clover, "lqcd_clover_export: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_clover_export: bad precision");
   CUDA_TRY(DISPATCH_PREC(prec, clover_export<double>(h->g, clover, canon, as_stream(stream)),
                          clover_export<float>(h->g, clover, canon, as_stream(stream))), "clover_export");
@@ -330,6 +357,7 @@ lqcd_status lqcd_clover_export(const lqcd_geom* h, const void* clover, void* can
 }
 lqcd_status lqcd_field_to_f32(const lqcd_geom* h, lqcd_field_kind kind, lqcd_recon recon, const void* src64, void* dst32, void* stream) {
   REQUIRE(h && src64 && dst32 && src64 != dst32, "lqcd_field_to_f32: NULL or aliased argument");
+  DeviceGuard dg(h);
   REQUIRE(kind == LQCD_FIELD_GAUGE || kind == LQCD_FIELD_SPINOR || kind == LQCD_FIELD_CLOVER, "lqcd_field_to_f32: bad kind");
   size_t n = lqcd_field_bytes(h, kind, LQCD_F64, recon) / sizeof(double2);
   CUDA_TRY(to_f32(src64, dst32, n, as_stream(stream)), "to_f32");
@@ -339,6 +367,8 @@ lqcd_status lqcd_field_to_f32(const lqcd_geom* h, lqcd_field_kind kind, lqcd_rec
 lqcd_status lqcd_clover_build(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, lqcd_recon recon, void* clover,
                               void* clover_inv, lqcd_prec out_prec, void* stream) {
   REQUIRE(h && d && U64 && clover, "lqcd_clover_build: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_clover_build: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(out_prec) && valid_recon(recon), "lqcd_clover_build: bad precision / recon");
   REQUIRE(clover != U64 && clover_inv != U64 && clover != clover_inv, "lqcd_clover_build: aliased buffers");
   UNSUPPORTED_ON_SLAB(h, "lqcd_clover_build (use lqcd_clover_build_slab)");
@@ -353,6 +383,8 @@ lqcd_status lqcd_clover_build_slab(const lqcd_geom* h, const lqcd_dirac* d, cons
                                    const void* halo_lo, const void* halo_hi, void* clover, void* clover_inv,
                                    lqcd_prec out_prec, void* stream) {
   REQUIRE(h && d && U64 && clover, "lqcd_clover_build_slab: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_clover_build_slab: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_clover_build_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
   REQUIRE((halo_lo || (h->g.edges & LQCD_SLAB_OPEN_LO)) && (halo_hi || (h->g.edges & (LQCD_SLAB_OPEN_HI | LQCD_SLAB_SF_HI))),
           "lqcd_clover_build_slab: a gauge halo is required on every face that is not an open boundary");
@@ -369,6 +401,7 @@ lqcd_status lqcd_clover_build_slab(const lqcd_geom* h, const lqcd_dirac* d, cons
 lqcd_status lqcd_dw_slab_pack(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* in, void* send_lo,
                               void* send_hi, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && U && in && send_lo && send_hi, "lqcd_dw_slab_pack: NULL argument");
+  DeviceGuard dg(h);
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_dw_slab_pack: the geometry is not a slab (bc != LQCD_BC_SLAB)");
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_slab_pack: bad precision / recon");
   REQUIRE(send_lo != send_hi, "lqcd_dw_slab_pack: aliased face buffers");
@@ -381,6 +414,8 @@ lqcd_status lqcd_dw_slab_pack(const lqcd_geom* h, const lqcd_dirac* d, const voi
 lqcd_status lqcd_dw_slab_faces(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* recv_lo,
                                const void* recv_hi, void* out, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && U && recv_lo && recv_hi && out, "lqcd_dw_slab_faces: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_dw_slab_faces: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_dw_slab_faces: the geometry is not a slab (bc != LQCD_BC_SLAB)");
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_slab_faces: bad precision / recon");
   CUDA_TRY(DISPATCH_PREC(prec, slab_faces<double>(h, d->kappa, dagger != 0, U, (int)recon, recv_lo, recv_hi, out, as_stream(stream)),
@@ -410,6 +445,8 @@ extern "C" {
 lqcd_status lqcd_dw_apply_multi(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
                                 void* out, int nrhs, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && U && in && out, "lqcd_dw_apply_multi: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_dw_apply_multi: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply_multi: bad precision / recon");
   REQUIRE(nrhs >= 1 && nrhs <= 64, "lqcd_dw_apply_multi: nrhs must be in 1..64");
   const size_t fb = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon);
@@ -424,6 +461,8 @@ lqcd_status lqcd_dw_apply_multi(const lqcd_geom* h, const lqcd_dirac* d, const v
 static lqcd_status dw_common(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
                              void* out, lqcd_prec prec, lqcd_recon recon, void* stream, bool dagger) {
   REQUIRE(h && d && U && in && out, "lqcd_dw_apply: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_dw_apply: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply: bad precision / recon");
   REQUIRE(out != in && out != U && out != clover, "lqcd_dw_apply: output aliases an input (PAPER.md:121: separate pso/psi)");
   CUDA_TRY(DISPATCH_PREC(prec, dw_apply_t<double>(h, d, U, clover, in, out, dagger, (int)recon, as_stream(stream)),
@@ -451,6 +490,8 @@ extern "C" {
 lqcd_status lqcd_dw_eo_apply(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* clover_inv,
                              const void* in_e, void* out_e, void* tmp, int dagger, lqcd_prec prec, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && U && clover && clover_inv && in_e && out_e && tmp, "lqcd_dw_eo_apply: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_dw_eo_apply: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_eo_apply: bad precision / recon");
   REQUIRE(out_e != in_e && tmp != in_e && tmp != out_e, "lqcd_dw_eo_apply: aliased buffers");
   REQUIRE(d->mu == 0.0, "lqcd_dw_eo_apply: the even-odd operator does not support a twisted mass (mu != 0)");
@@ -463,6 +504,7 @@ lqcd_status lqcd_dw_eo_apply(const lqcd_geom* h, const lqcd_dirac* d, const void
 
 lqcd_status lqcd_point_source(const lqcd_geom* h, const int y[4], int spin, int colour, void* b, lqcd_prec prec, void* stream) {
   REQUIRE(h && y && b, "lqcd_point_source: NULL argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_point_source: bad precision");
   REQUIRE(spin >= 0 && spin < 4 && colour >= 0 && colour < 3, "lqcd_point_source: bad spin/colour");
   for (int i = 0; i < 4; i++) REQUIRE(y[i] >= 0 && y[i] < h->g.L[i], "lqcd_point_source: position outside the lattice");
@@ -473,6 +515,7 @@ lqcd_status lqcd_point_source(const lqcd_geom* h, const int y[4], int spin, int 
 
 lqcd_status lqcd_spinor_norm2(const lqcd_geom* h, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream) {
   REQUIRE(h && v && workspace && result_host, "lqcd_spinor_norm2: NULL argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_spinor_norm2: bad precision");
   size_t n = spinor_complex(h->g) / (half ? 2 : 1);
   double* partial = (double*)workspace;
@@ -484,6 +527,7 @@ lqcd_status lqcd_spinor_norm2(const lqcd_geom* h, const void* v, int half, lqcd_
 lqcd_status lqcd_correlator_ps(const lqcd_geom* h, const void* columns, int ncol, lqcd_prec prec, void* workspace,
                                double* C_host, void* stream) {
   REQUIRE(h && columns && workspace && C_host, "lqcd_correlator_ps: NULL argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec) && ncol >= 1 && ncol <= 4096, "lqcd_correlator_ps: bad precision or column count");
   const Geom& g = h->g;
   double* partial = (double*)workspace;   // the workspace is several spinor fields large: ntiles*b3 + L4 doubles fit
@@ -497,6 +541,7 @@ lqcd_status lqcd_correlator_ps(const lqcd_geom* h, const void* columns, int ncol
 }
 lqcd_status lqcd_spinor_dot(const lqcd_geom* h, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream) {
   REQUIRE(h && u && v && workspace && result_host, "lqcd_spinor_dot: NULL argument");
+  DeviceGuard dg(h);
   REQUIRE(valid_prec(prec), "lqcd_spinor_dot: bad precision");
   size_t n = spinor_complex(h->g) / (half ? 2 : 1);
   double* partial = (double*)workspace;
@@ -609,6 +654,8 @@ extern "C" {
 lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b, void* x,
                           void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && f && b && x && workspace && parm && info, "lqcd_cg_solve: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_cg_solve: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(valid_recon(recon), "lqcd_cg_solve: bad recon");
   REQUIRE(f->U64, "lqcd_cg_solve: U64 is required");
   REQUIRE(x != b, "lqcd_cg_solve: x aliases b");
@@ -642,6 +689,14 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
   if (!parm->eo) {
     Op<double> M = make_op<double>(c, nullptr);
     void* bp = c.v64[4];
+    if (g.bc != LQCD_BC_PERIODIC) {
+      // D7: the solve lives on the interior; components of b on frozen slices are ignored (as in the even-odd branch),
+      // so that |b| and b - Dx below do not count them
+      void* bm = c.v64[6];
+      CKS(cudaMemcpyAsync(bm, b, nfull * sizeof(double2), cudaMemcpyDeviceToDevice, s), "copy b");
+      CKS(mask_frozen<double>(g, bm, s), "mask");
+      b = bm;
+    }
     CKS(M.apply(b, bp, true, EPI_STORE, nullptr, nullptr, nullptr, nullptr, s), "D^+ b");
     st = solve_normal(c, bp, x, &iters, &outer, &rho0);
     if (st != LQCD_OK && st != LQCD_ENOTCONV) { info->iters = iters; info->outer = outer; return st; }
@@ -794,6 +849,8 @@ extern "C" lqcd_status lqcd_cg_solve_slab(const lqcd_geom* h, const lqcd_dirac* 
                                           void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info,
                                           const lqcd_slab_comm* comm, lqcd_recon recon, void* stream) {
   REQUIRE(h && d && f && b && x && workspace && parm && info && comm, "lqcd_cg_solve_slab: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_cg_solve_slab: kappa must be positive and finite (got %g)", d->kappa);
+  DeviceGuard dg(h);
   REQUIRE(h->g.bc == LQCD_BC_SLAB, "lqcd_cg_solve_slab: the geometry is not a slab (bc != LQCD_BC_SLAB)");
   REQUIRE(valid_recon(recon), "lqcd_cg_solve_slab: bad recon");
   REQUIRE(f->U64, "lqcd_cg_solve_slab: U64 is required");
@@ -882,6 +939,7 @@ extern "C" {
 lqcd_status lqcd_propagator(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4], void* columns,
                             void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info infos[12], lqcd_recon recon, void* stream) {
   REQUIRE(h && d && f && y && columns && workspace && parm && infos, "lqcd_propagator: NULL argument");
+  DeviceGuard dg(h);
   const size_t sbytes = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, LQCD_F64, recon);
   // the source lives in the last fp64 workspace vector, which lqcd_cg_solve does not touch
   void* b = (char*)workspace + (size_t)(WS_SPINORS64 - 1) * align256(sbytes);

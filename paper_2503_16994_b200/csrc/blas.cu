@@ -8,10 +8,14 @@ namespace lqcd {
 template <typename T> using T2 = typename vec2<T>::type;
 
 static const int RB_THREADS = 256;
+// SMs of the device the geometry was created on (lqcd_geom_create); 148 = B200 until a geometry exists
+static int g_reduce_sms = 148;
+void set_reduce_sm_count(int sms) { if (sms > 0) g_reduce_sms = sms; }
+int reduce_blocks_max() { return g_reduce_sms * 8; }
 int reduce_blocks(size_t ncomplex) {
   size_t b = (ncomplex + (size_t)RB_THREADS * 8 - 1) / ((size_t)RB_THREADS * 8);
   if (b < 1) b = 1;
-  if (b > 148 * 8) b = 148 * 8;
+  if (b > (size_t)reduce_blocks_max()) b = (size_t)reduce_blocks_max();
   return (int)b;
 }
 

@@ -802,13 +802,10 @@ static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
 
 template <typename T, int RECON, int DIAG>
 static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg& c, cudaStream_t s) {
-  static size_t attr_smem = 0;   // the attribute is per function; raise it when a launch needs more
-  if (c.smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(dw_pipe_kernel<T, RECON, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)c.smem);
-    if (e != cudaSuccess) return e;
-    attr_smem = c.smem;
-  }
+  // the attribute is per function AND per device: set it on every launch (a host-side call of about a microsecond) rather
+  // than cache it in a process-wide variable that another device or thread would not see
+  cudaError_t e = cudaFuncSetAttribute(dw_pipe_kernel<T, RECON, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
   dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, a, c.nslot);
   count_launch();
   return cudaGetLastError();
@@ -831,14 +828,16 @@ static DirectCfg direct_config_t(const Geom& g, int parity) {
   const int items = c.kind == KIND_SPLIT ? 2 * g.ntiles : g.ntiles;
   c.grid = items;
   if (mode == MODE_DIRECT) return c;
-  static int per_sm[3] = {0, 0, 0};   // resident CTAs per SM of this instantiation, by kernel kind
-  int& occ = per_sm[c.kind];
-  if (occ == 0) {
+  // resident CTAs per SM of this instantiation on the current device for this CTA size (queried per call: the
+  // answer depends on the device and on c.threads, and the query is a host-side table lookup)
+  int occ = 0;
+  {
     cudaError_t e;
     if (c.kind == KIND_FULL) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel<T, RECON, DIAG>, c.threads, 0);
     else if (c.kind == KIND_HALF) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel_h<T, RECON, DIAG, false>, c.threads, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dw_kernel_h<T, RECON, DIAG, true>, c.threads, 0);
     if (e != cudaSuccess || occ < 1) occ = 1;
+    if (occ > 8) occ = 8;   // partial_len() (api.cu) sizes the per-CTA partial sums for at most 8 CTAs per SM
   }
   int ctas = env_int("LQCD_CTAS_PER_SM", occ);
   if (ctas < 1 || ctas > occ) ctas = occ;

@@ -40,6 +40,8 @@ struct CgState {
   int pad;
 };
 int reduce_blocks(size_t ncomplex);  // grid size used by the norm/dot kernels (partial buffer length)
+int reduce_blocks_max();             // its upper bound: 8 CTAs per SM of the device
+void set_reduce_sm_count(int sms);   // called by lqcd_geom_create with the device's SM count
 template <typename T> cudaError_t norm2_partial(const void* v, size_t ncomplex, double* partial, cudaStream_t s);
 template <typename T> cudaError_t dot_partial(const void* u, const void* v, size_t ncomplex, double* partial, cudaStream_t s);
 cudaError_t final_sum(const double* partial, int n, int nvals, double* result, cudaStream_t s);

@@ -113,3 +113,17 @@ def site_rel_err(got, ref, mask=None):
 def round_f32(a):
     """R14: the fp32 path's inputs, rounded once, promoted back to fp64 for the oracle."""
     return a.astype(np.complex64).astype(np.complex128)
+
+
+def f32_storage_err(got32, ref64, build_tol=2e-14):
+    """fp32 storage of a field built in fp64 (R14: built in fp64, rounded once).  The library's fp64 value agrees with
+    the oracle's to build_tol, so the stored fp32 number is the rounding of a value within build_tol of ref64: its
+    distance from ref64 is at most half an fp32 spacing at |ref64| plus build_tol.  Returns the worst excess over
+    that bound (<= 0 means every element is a correct rounding); the same rule is used by every test of an fp32 clover
+    term (whole lattice and slabs)."""
+    worst = -np.inf
+    for part in (np.real, np.imag):
+        g, r = part(got32).astype(np.float64), part(ref64).astype(np.float64)
+        half = 0.5 * np.spacing(np.abs(r).astype(np.float32)).astype(np.float64)
+        worst = max(worst, float(np.max(np.abs(g - r) - half - build_tol)))
+    return worst

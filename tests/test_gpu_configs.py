@@ -1,0 +1,233 @@
+"""-m gpu parity at the STATED size of BASELINE.json's configs 2, 3 and 5b (SURVEY.md 8(d) protocols 2, 3, 5; config 1
+is tests/test_gpu_dw.py::test_config1_4to4_haar_fp64, config 4's 4^3 x 8 sub-run tests/test_gpu_cg.py and
+tests/test_gpu_dw.py, config 5a tests/test_gpu_fullsize.py).
+
+  config 2  16^3 x 32 periodic, kappa = 0.135, csw = 1.7: one Dw and one Dw^+ against the full-size oracle, element by
+            element, fp64 (1e-12) and fp32 (2e-6, the oracle consuming the inputs rounded once: R14).
+  config 3  24^3 x 48 open, kappa = 0.1365, csw = 1.9: point-source columns solved on the GPU,
+            pin P9 through two applications of the ORACLE operator per column (normal-equation residual <= 2 tol);
+            the full oracle CG on the 8^3 x 16 open sub-run with the same kappa / csw, plain and even-odd + mixed.
+  config 5b 64^3 x 128 periodic, kappa = 0.137, csw = 1.9: D and D^+ through the kernel bench.py times, on 4096 seeded
+            random sites plus the 16 lattice corners against oracle.dw_at_sites.  The oracle reads only the 3^4
+            neighbourhood of a site, so only those entries of the device fields are downloaded into (lazily
+            allocated, otherwise zero) full-size host arrays -- a wrong index on the oracle side reads zeros and fails.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2503_16994_b200 import binding as B
+from paper_2503_16994_b200 import synth
+
+from gpu_util import Lattice, interior, round_f32, site_rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL = {B.F64: 1e-12, B.F32: 2e-6}
+
+
+# ---------------------------------------------------------------------------------------------------- config 2
+@pytest.fixture(scope="module")
+def config2():
+    L, kappa, csw = (16, 16, 16, 32), 0.135, 1.7
+    U = synth.smooth_gauge(L, synth.seed_for(2, 0))
+    psi = synth.gaussian_spinor(L, synth.seed_for(2, 1))
+    A = oracle.clover_blocks(L, U, kappa, csw)   # built in fp64 from the fp64 links (R14)
+    lat = Lattice(L)
+    lat.set_gauge(U, recons=(B.RECON_18, B.RECON_12), precs=(B.F64, B.F32))
+    lat.build_clover(kappa, csw, precs=(B.F64, B.F32))
+    yield dict(L=L, kappa=kappa, U=U, psi=psi, A=A, lat=lat)
+    lat.close()
+
+
+@pytest.mark.parametrize("prec,recon", [(B.F64, B.RECON_18), (B.F64, B.RECON_12), (B.F32, B.RECON_18), (B.F32, B.RECON_12)])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_config2_16x16x16x32_full_oracle(config2, prec, recon, dagger):
+    c = config2
+    L, lat = c["L"], c["lat"]
+    assert "dw_pipe_kernel" in B.dw_plan(lat.g, prec, recon, True)   # the kernel bench.py's config-2 row times
+    if prec == B.F64:
+        ref = oracle.dw(L, c["U"], c["psi"], c["kappa"], c["A"], dagger=dagger)
+    else:   # R14: links, clover blocks and spinor rounded once to fp32, promoted back for the oracle
+        ref = oracle.dw(L, round_f32(c["U"]), round_f32(c["psi"]), c["kappa"], round_f32(c["A"]), dagger=dagger)
+    got = lat.dw(c["kappa"], c["psi"], prec=prec, recon=recon, dagger=dagger)
+    assert site_rel_err(got, ref) <= TOL[prec]
+
+
+# ---------------------------------------------------------------------------------------------------- config 3
+def _open_setup(L, kappa, csw, seed, dev_gen):
+    if dev_gen:   # 2.6 M links: drawn on the device, downloaded for the oracle (never two generators)
+        Ud = synth.smooth_gauge_torch(L, seed, torch.device("cuda", torch.cuda.current_device()))
+        U = Ud.cpu().numpy()
+    else:
+        U = synth.smooth_gauge(L, seed)
+        Ud = U
+    lat = Lattice(L, B.BC_OPEN)
+    lat.set_gauge(Ud, precs=(B.F64, B.F32))
+    lat.build_clover(kappa, csw, precs=(B.F64, B.F32), inverse=True)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=B.BC_OPEN)
+    return U, A, lat
+
+
+def _solve(lat, kappa, b_canon, tol, eo_mixed):
+    b = lat.spinor(b_canon)
+    x = lat.alloc(B.FIELD_SPINOR)
+    ws = lat.alloc(B.FIELD_WORKSPACE)
+    kw = {}
+    if eo_mixed:
+        kw = dict(eo=True, mixed=True, U32=lat.U[(B.F32, 18)], clover32=lat.A[B.F32], clover_inv32=lat.Ainv[B.F32])
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], b, x, ws, tol=tol, maxiter=10000,
+                      clover_inv64=lat.Ainv[B.F64], **kw)
+    return lat.spinor_to_host(x), info
+
+
+def test_config3_24x24x24x48_open_p9():
+    """P9 at the stated size: the ORACLE operator's residuals of GPU solutions (two oracle applications per column).
+    Plain fp64 CG stops on the normal-equation residual of D itself, so that residual is <= 2 tol through the oracle;
+    the even-odd + mixed solver stops on the normal-equation residual of the preconditioned operator D^ (D8), which
+    is checked through oracle.dhat on the even sites, and its full-system true residual is bounded as in P10."""
+    L, kappa, csw, tol = (24, 24, 24, 48), 0.1365, 1.9, 1e-10
+    U, A, lat = _open_setup(L, kappa, csw, synth.seed_for(3, 0), dev_gen=True)
+    Ainv = oracle.clover_inverse(L, A)
+    y = (0, 0, 0, L[3] // 2)   # R12
+    frozen = ~interior(L, B.BC_OPEN)
+    bc = B.BC_OPEN
+    for col in (0, 7):
+        b = synth.point_source(L, y, col // 3, col % 3)
+        bp = oracle.dw(L, U, b, kappa, A, bc=bc, dagger=True)
+        x, info = _solve(lat, kappa, b, tol, eo_mixed=False)
+        assert info["status"] == B.OK
+        r = b - oracle.dw(L, U, x, kappa, A, bc=bc)
+        rn = np.linalg.norm(oracle.dw(L, U, r, kappa, A, bc=bc, dagger=True)) / np.linalg.norm(bp)
+        assert rn <= 2 * tol, (col, rn)
+        assert abs(info["rel_resid_true"] - np.linalg.norm(r)) <= 0.5 * np.linalg.norm(r) + 1e-13
+        assert np.all(x[frozen] == 0)
+        x_plain = x
+        # even-odd + mixed precision (the bench's second propagator row)
+        x, info = _solve(lat, kappa, b, tol, eo_mixed=True)
+        assert info["status"] == B.OK
+        par = synth_parity(L)
+        xe = np.where(par[:, None, None] == 0, x, 0)
+        # b^_e = b_e + kappa H_eo A_oo^-1 b_o; the source sits on an even site, so b^ = b
+        assert par[synth.site_index(L, y)] == 0
+        re = b - oracle.dhat(L, U, xe, kappa, A, Ainv, bc=bc)
+        re[par == 1] = 0
+        bph = oracle.dhat(L, U, b, kappa, A, Ainv, bc=bc, dagger=True)
+        rnh = np.linalg.norm(oracle.dhat(L, U, re, kappa, A, Ainv, bc=bc, dagger=True)) / np.linalg.norm(bph)
+        assert rnh <= 2 * tol, (col, rnh)
+        rt = np.linalg.norm(b - oracle.dw(L, U, x, kappa, A, bc=bc))
+        assert abs(info["rel_resid_true"] - rt) <= 0.5 * rt + 1e-13
+        # both solvers solve the same system: the solutions agree to cond * residual
+        assert np.linalg.norm(x - x_plain) / np.linalg.norm(x_plain) <= 1e-6, (col, rt)
+        assert np.all(x[frozen] == 0)
+    lat.close()
+
+
+def synth_parity(L):
+    n = np.arange(synth.vol(L))
+    p = np.zeros_like(n)
+    for mu in range(4):
+        p += n % L[mu]
+        n = n // L[mu]
+    return p & 1
+
+
+@pytest.mark.parametrize("eo_mixed", [False, True])
+def test_config3_subrun_8x8x8x16_open_oracle_cg(eo_mixed):
+    """The full oracle CG on the 8^3 x 16 open sub-run of config 3 (same kappa, csw, tolerance)."""
+    L, kappa, csw, tol = (8, 8, 8, 16), 0.1365, 1.9, 1e-10
+    U, A, lat = _open_setup(L, kappa, csw, synth.seed_for(3, 0), dev_gen=False)
+    y = (0, 0, 0, L[3] // 2)
+    for col in (0, 5, 10):
+        b = synth.point_source(L, y, col // 3, col % 3)
+        xo, it_o, rn_o, rt_o = oracle.cg(L, U, b, kappa, A, bc=B.BC_OPEN, tol=tol)
+        assert it_o > 0
+        x, info = _solve(lat, kappa, b, tol, eo_mixed)
+        assert info["status"] == B.OK
+        assert np.linalg.norm(x - xo) / np.linalg.norm(xo) <= 1e-8
+        if not eo_mixed:
+            assert abs(info["iters"] - it_o) <= 2
+        assert np.all(x[~interior(L, B.BC_OPEN)] == 0)
+    lat.close()
+
+
+# ---------------------------------------------------------------------------------------------------- config 5b
+def _neighbourhood(L, sites):
+    """Canonical indices of all sites within one step in every direction (the 3^4 box) of the given sites: what
+    oracle.dw_at_sites reads (hops: x +- mu; clover leaves: links at x, x +- mu, x +- nu, x +- mu +- nu)."""
+    L = [int(v) for v in L]
+    s = np.asarray(sites, dtype=np.int64)
+    x = np.empty((len(s), 4), dtype=np.int64)
+    n = s.copy()
+    for mu in range(4):
+        x[:, mu] = n % L[mu]
+        n //= L[mu]
+    offs = np.array([[a, b, c, d] for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1) for d in (-1, 0, 1)])
+    nb = (x[:, None, :] + offs[None, :, :]) % np.array(L)[None, None, :]
+    idx = nb[..., 0] + L[0] * (nb[..., 1] + L[1] * (nb[..., 2] + L[2] * nb[..., 3]))
+    return np.unique(idx.reshape(-1))
+
+
+def test_config5b_64x64x64x128_sampled():
+    L, kappa, csw = (64, 64, 64, 128), 0.137, 1.9
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120 * (1 << 30):
+        pytest.skip("needs ~110 GB of device memory, %d GB free" % (free >> 30))
+    V = synth.vol(L)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    rng = np.random.Generator(np.random.PCG64(synth.seed_for(5, 9)))
+    sites = list(rng.integers(0, V, size=4096))
+    for c in range(16):
+        sites.append(synth.site_index(L, [(L[mu] - 1) if (c >> mu) & 1 else 0 for mu in range(4)]))
+    sites = np.array(sorted(set(int(s) for s in sites)), dtype=np.int64)
+    nb = _neighbourhood(L, sites)
+    nb_d = torch.from_numpy(nb).to(dev)
+    g = B.geom_create(L)
+    Uc = synth.smooth_gauge_torch(L, synth.seed_for(5, 0), dev)
+    U_host = np.zeros((V, 4, 3, 3), dtype=np.complex128)   # untouched pages stay unmapped zeros
+    U_host[nb] = Uc[nb_d].cpu().numpy()
+    U = B.alloc_field(g, B.FIELD_GAUGE)
+    B.gauge_import(g, Uc, U)
+    torch.cuda.synchronize()
+    del Uc
+    torch.cuda.empty_cache()
+    A = B.alloc_field(g, B.FIELD_CLOVER)
+    B.clover_build(g, kappa, csw, U, A)
+    psic = synth.gaussian_spinor_torch(L, synth.seed_for(5, 1), dev)
+    psi_host = np.zeros((V, 4, 3), dtype=np.complex128)
+    psi_host[nb] = psic[nb_d].cpu().numpy()
+    src, dst = B.alloc_field(g, B.FIELD_SPINOR), B.alloc_field(g, B.FIELD_SPINOR)
+    B.spinor_import(g, psic, src)
+    torch.cuda.synchronize()
+    canon = psic   # reuse the canonical buffer for the export
+    sites_d = torch.from_numpy(sites).to(dev)
+    for prec in (B.F64, B.F32):
+        if prec == B.F32:   # round the resident fields once (R14); the oracle gets the same rounded arrays
+            U32, A32, s32 = (B.alloc_field(g, k, B.F32) for k in (B.FIELD_GAUGE, B.FIELD_CLOVER, B.FIELD_SPINOR))
+            B.field_to_f32(g, B.FIELD_GAUGE, B.RECON_18, U, U32)
+            B.clover_build(g, kappa, csw, U, A32, None, B.RECON_18, B.F32)
+            B.field_to_f32(g, B.FIELD_SPINOR, B.RECON_18, src, s32)
+            torch.cuda.synchronize()
+            del U, A, src, dst
+            torch.cuda.empty_cache()
+            U, A, src, dst = U32, A32, s32, B.alloc_field(g, B.FIELD_SPINOR, B.F32)
+            psi_host[nb] = round_f32(psi_host[nb])
+        assert "dw_pipe_kernel" in B.dw_plan(g, prec, B.RECON_18, True)
+        for dagger, fn in ((False, B.dw_apply), (True, B.dwdag_apply)):
+            dst.fill_(0x7F)
+            fn(g, kappa, U, A, src, dst, prec, B.RECON_18)
+            B.spinor_export(g, dst, canon, prec)
+            torch.cuda.synchronize()
+            got = canon[sites_d].cpu().numpy()
+            # fp32: links rounded once; the clover term is built in fp64 from the fp64 links and then rounded (R14),
+            # which the site-sampled oracle (clover on the fly) sees as fp64 -- a 6e-8 relative difference in A
+            Uo = U_host
+            if prec == B.F32:
+                Uo = np.zeros_like(U_host)
+                Uo[nb] = round_f32(U_host[nb])
+            ref = oracle.dw_at_sites(L, Uo, psi_host, sites, kappa, csw, dagger=dagger)
+            err = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(ref.reshape(len(sites), -1), axis=1)
+            assert err.max() <= TOL[prec], (prec, dagger, err.max())
+            del Uo
+    B.geom_destroy(g)

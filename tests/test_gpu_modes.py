@@ -137,3 +137,71 @@ def test_dw_apply_multi(mode, prec):
     with pytest.raises(B.LqcdError):   # overlapping arrays
         B.dw_apply_multi(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src, src[fb:], 2, prec)
     lat.close()
+
+
+def test_kappa_must_be_positive():
+    """kappa <= 0 (or not finite) is refused by every operator / solver entry point instead of producing NaN on the
+    pipeline kernel (which folds the diagonal term in as -(1/kappa) A psi) and A psi on the others."""
+    L = (4, 4, 4, 4)
+    U, psi = inputs(L, B.BC_PERIODIC, 91)
+    lat = Lattice(L)
+    lat.set_gauge(U)
+    lat.build_clover(0.125, 1.0)
+    src, dst = lat.spinor(psi), lat.alloc(B.FIELD_SPINOR)
+    ws = lat.alloc(B.FIELD_WORKSPACE)
+    for kappa in (0.0, -0.1, float("inf"), float("nan")):
+        with pytest.raises(B.LqcdError) as e:
+            B.dw_apply(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, dst)
+        assert e.value.status == B.EINVAL
+        with pytest.raises(B.LqcdError) as e:
+            B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, dst, ws)
+        assert e.value.status == B.EINVAL
+    lat.close()
+
+
+@pytest.mark.parametrize("mode", ["split", "stream"], indirect=True)
+def test_cg_partial_buffer_split_grid(mode):
+    """16x16x16x6: tiles of 64 sites per parity and 192 tiles, so that dw_mode = split launches 2 * ntiles = 384 CTAs,
+    each writing one partial sum of the fused CG epilogues -- more than ntiles and more than the BLAS-1 grids; the
+    workspace's partial-sum buffer has to hold them (the solution is compared with the oracle's CG)."""
+    L, kappa, csw = (16, 16, 16, 6), 0.13, 1.5
+    U, _ = inputs(L, B.BC_PERIODIC, 95)
+    A = oracle.clover_blocks(L, U, kappa, csw)
+    lat = Lattice(L)
+    lat.set_gauge(U)
+    lat.build_clover(kappa, csw)
+    b = synth.point_source(L, (3, 2, 1, 4), 2, 1)
+    xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, tol=1e-10)
+    x, ws = lat.alloc(B.FIELD_SPINOR), lat.alloc(B.FIELD_WORKSPACE)
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], lat.spinor(b), x, ws, tol=1e-10)
+    assert abs(info["iters"] - it_o) <= 2
+    xg = lat.spinor_to_host(x)
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= 1e-8
+    lat.close()
+
+
+@pytest.mark.parametrize("eo", [False, True])
+def test_cg_source_on_frozen_slice_is_ignored(eo):
+    """D7: the solve lives on the interior.  Components of b on frozen slices are ignored by both solver branches: a
+    source with support on the frozen slice as well gives the solution and the residuals of its interior part."""
+    L, bc, kappa, csw = (4, 4, 4, 8), B.BC_OPEN, 0.13, 1.5
+    U, _ = inputs(L, bc, 97)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
+    lat = Lattice(L, bc)
+    lat.set_gauge(U)
+    lat.build_clover(kappa, csw, inverse=True)
+    b_in = synth.point_source(L, (1, 2, 3, 4), 0, 1)
+    b = b_in + 5.0 * synth.point_source(L, (0, 1, 0, 0), 3, 2) + 2.0 * synth.point_source(L, (2, 1, 0, L[3] - 1), 1, 0)
+    xo, _, _, rt_o = oracle.cg(L, U, b_in, kappa, A, bc=bc, tol=1e-10)
+    x, ws = lat.alloc(B.FIELD_SPINOR), lat.alloc(B.FIELD_WORKSPACE)
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], lat.spinor(b), x, ws, tol=1e-10,
+                      clover_inv64=lat.Ainv[B.F64], eo=eo)
+    xg = lat.spinor_to_host(x)
+    assert np.linalg.norm(xg - xo) / np.linalg.norm(xo) <= 1e-8
+    assert info["rel_resid_true"] <= 50e-10
+    # a source living on frozen slices only: x = 0, converged at once
+    bz = synth.point_source(L, (0, 1, 0, 0), 3, 2)
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], lat.spinor(bz), x, ws, tol=1e-10,
+                      clover_inv64=lat.Ainv[B.F64], eo=eo)
+    assert info["iters"] == 0 and torch.count_nonzero(x).item() == 0
+    lat.close()
