@@ -87,27 +87,39 @@ static void choose_tiling(Geom& g) {
   for (int i = 1; i < 4; i++) g.lb[i] = ilog2(b[i]);
   g.TV = (b[0] / 2) * b[1] * b[2] * b[3];
   g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
-  // L2 chunking: sweep time inside a chunk of (c1 x c2) tiles in (x2, x3) so that one time layer of the chunk
-  // (the reuse distance of a time-neighbour) stays well inside L2; cut as few faces as possible.
+  // L2 chunking: sweep direction sw inside a chunk of (c1 x c2) tiles along (da, db) so that one layer of the chunk
+  // (the reuse distance of a neighbour in the sweep direction) stays well inside L2.  Chunk borders cut the faces of da
+  // and db: a cut face is gathered from DRAM a second time, in whole 128-byte lines.  With the site order inside a
+  // tile (lqcd_internal.cuh) the x3 and x4 faces are contiguous runs of >= 128 bytes while an x2 face uses a quarter of
+  // every line it touches, so the default sweeps x2 (direction 1) and chunks (x3, x4); cut as few faces as possible.
+  int sw = 1;
+  if (getenv("LQCD_SWEEP")) {
+    const int e = atoi(getenv("LQCD_SWEEP"));
+    if (e >= 1 && e <= 3) sw = e;
+  }
+  g.sw = sw;
+  g.da = sw == 1 ? 2 : 1;
+  g.db = sw == 3 ? 2 : 3;
   long budget = 32768;
   if (getenv("LQCD_LAYER_SITES")) budget = atol(getenv("LQCD_LAYER_SITES"));
   int best1 = 1, best2 = 1;
   double best_cost = 1e30;
   long best_sites = 0;
-  for (int c1 = 1; c1 <= g.nt[1]; c1++) {
-    if (g.nt[1] % c1) continue;
-    for (int c2 = 1; c2 <= g.nt[2]; c2++) {
-      if (g.nt[2] % c2) continue;
-      long sites = (long)g.L[0] * c1 * b[1] * c2 * b[2] * b[3];
+  const int na = g.nt[g.da], nb = g.nt[g.db];
+  for (int c1 = 1; c1 <= na; c1++) {
+    if (na % c1) continue;
+    for (int c2 = 1; c2 <= nb; c2++) {
+      if (nb % c2) continue;
+      long sites = (long)g.L[0] * c1 * b[g.da] * c2 * b[g.db] * b[sw];
       if (sites > budget && !(c1 == 1 && c2 == 1)) continue;
-      double cost = (c1 < g.nt[1] ? 1.0 / (c1 * b[1]) : 0.0) + (c2 < g.nt[2] ? 1.0 / (c2 * b[2]) : 0.0);
+      double cost = (c1 < na ? 1.0 / (c1 * b[g.da]) : 0.0) + (c2 < nb ? 1.0 / (c2 * b[g.db]) : 0.0);
       if (cost < best_cost - 1e-12 || (fabs(cost - best_cost) <= 1e-12 && sites > best_sites)) {
         best_cost = cost; best_sites = sites; best1 = c1; best2 = c2;
       }
     }
   }
   int ce[2];
-  if (parse_ints(getenv("LQCD_CHUNK"), ce, 2) && ce[0] >= 1 && ce[1] >= 1 && g.nt[1] % ce[0] == 0 && g.nt[2] % ce[1] == 0) {
+  if (parse_ints(getenv("LQCD_CHUNK"), ce, 2) && ce[0] >= 1 && ce[1] >= 1 && na % ce[0] == 0 && nb % ce[1] == 0) {
     best1 = ce[0]; best2 = ce[1];
   }
   g.c1 = best1;
@@ -271,6 +283,12 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
       cudaFree(dtab); free(h); return LQCD_ECUDA;
     }
     g.tile_tab = dtab;
+    unsigned int* sched = nullptr;
+    if (!cuda_ok(cudaMalloc(&sched, SCHED_SLOTS * 2 * sizeof(unsigned int)), "cudaMalloc(scheduler)") ||
+        !cuda_ok(cudaMemset(sched, 0, SCHED_SLOTS * 2 * sizeof(unsigned int)), "cudaMemset(scheduler)")) {
+      cudaFree(sched); cudaFree(dtab); free(h); return LQCD_ECUDA;
+    }
+    g.sched = sched;
   }
   *out = h;
   return LQCD_OK;
@@ -280,6 +298,7 @@ lqcd_status lqcd_geom_destroy(lqcd_geom* g) {
   if (g) {
     DeviceGuard dg(g);
     if (g->g.tile_tab) cudaFree((void*)g->g.tile_tab);
+    if (g->g.sched) cudaFree((void*)g->g.sched);
     free(g);
   }
   return LQCD_OK;

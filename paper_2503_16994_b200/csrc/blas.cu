@@ -213,22 +213,22 @@ template <typename T> cudaError_t dot_partial(const void* u, const void* v, size
   return cudaGetLastError();
 }
 cudaError_t final_sum(const double* partial, int n, int nvals, double* result, cudaStream_t s) {
-  final_sum_kernel<<<1, 256, 0, s>>>(partial, n, nvals, result);
+  final_sum_kernel<<<1, 1024, 0, s>>>(partial, n, nvals, result);
   count_launch();
   return cudaGetLastError();
 }
 cudaError_t cg_init_state(CgState* st, const double* partial, int n, double tol, cudaStream_t s) {
-  cg_init_kernel<<<1, 256, 0, s>>>(st, partial, n, tol);
+  cg_init_kernel<<<1, 1024, 0, s>>>(st, partial, n, tol);
   count_launch();
   return cudaGetLastError();
 }
 cudaError_t cg_reduce_alpha(CgState* st, const double* partial, int n, cudaStream_t s) {
-  cg_alpha_kernel<<<1, 256, 0, s>>>(st, partial, n);
+  cg_alpha_kernel<<<1, 1024, 0, s>>>(st, partial, n);
   count_launch();
   return cudaGetLastError();
 }
 cudaError_t cg_reduce_beta(CgState* st, const double* partial, int n, cudaStream_t s) {
-  cg_beta_kernel<<<1, 256, 0, s>>>(st, partial, n);
+  cg_beta_kernel<<<1, 1024, 0, s>>>(st, partial, n);
   count_launch();
   return cudaGetLastError();
 }

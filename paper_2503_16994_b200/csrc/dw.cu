@@ -15,6 +15,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
+
 #include "dw.cuh"
 #include "pipe.cuh"
 
@@ -369,12 +371,41 @@ struct CloverStage<T, C0, 0> {
 // With both fixed at compile time every shared-memory access of the arithmetic warps is an immediate offset from
 // one base register, and the two halo buffers interleave into rows of 2*PIPE_NF = PIPE_TV columns, i.e. halo rows
 // have the same stride as tile rows and a hop needs no stride select.
-enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12, PIPE_TV = 128, PIPE_NF = 64 };
+enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12, PIPE_TV = 128, PIPE_NF = 64,
+       PIPE_TQ = 4 };
 struct PipeBars {
   uint64_t full_sp, empty_sp;
   uint64_t full_h[2], empty_h[2];
   uint64_t full[PIPE_MAX_SLOTS], empty[PIPE_MAX_SLOTS];
+  uint64_t tq_full[PIPE_TQ], tq_empty[PIPE_TQ];   // tile queue: the producer lane tells the other warps which tile is next
+  int tq[PIPE_TQ];
 };
+
+// ---- tile scheduler ------------------------------------------------------------------------------------------
+// A CTA starts with tile blockIdx.x and then draws tiles gridDim.x, gridDim.x + 1, ... from a global counter
+// (DwArgs::sched[0]), so that at any moment the CTAs of the grid work on (nearly) consecutive tile indices no matter
+// how their speeds differ: with a static assignment b, b + grid, ... the CTAs drift apart over the hundreds of tiles
+// each of them walks, and the neighbour tiles a halo gathers are no longer the ones that just went through L2.
+// Only the producer lane draws; it hands every tile index to the halo and arithmetic warps through a small
+// shared-memory queue (negative index: no more tiles).
+__device__ __forceinline__ void tq_push(PipeBars* bars, const int kt, const int tile) {
+  const int q = kt & (PIPE_TQ - 1);
+  mbar_wait_relaxed(&bars->tq_empty[q], (uint32_t)(((kt / PIPE_TQ) & 1) ^ 1));
+  *(volatile int*)&bars->tq[q] = tile;
+  mbar_arrive(&bars->tq_full[q]);   // release: the index is visible to whoever sees the phase complete
+}
+__device__ __forceinline__ int tq_pop(PipeBars* bars, const int kt, const int lane) {
+  const int q = kt & (PIPE_TQ - 1);
+  mbar_wait(&bars->tq_full[q], (uint32_t)((kt / PIPE_TQ) & 1));
+  const int tile = *(volatile int*)&bars->tq[q];
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&bars->tq_empty[q]);
+  return tile;
+}
+__device__ __forceinline__ int next_tile(const Geom& g, unsigned int* sched, const int tile) {
+  const int n = sched ? (int)(gridDim.x + atomicAdd(sched, 1u)) : tile + (int)gridDim.x;
+  return n < g.ntiles ? n : -1;
+}
 
 struct RingPos {
   int slot;
@@ -513,7 +544,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   constexpr int NCU = (RECON == 12) ? 6 : 9;
   constexpr int NSTC = (DIAG == DIAG_PRE) ? 36 / NCU : 0;   // clover stages per tile
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ double s_red[PIPE_THREADS / 32];
+  __shared__ double s_red[2][PIPE_CONS_WARPS];
   if (a.skip != nullptr && *a.skip != 0) return;  // CG finished: uniform early exit
   constexpr int TV = PIPE_TV;
   const int tid = threadIdx.x;
@@ -534,6 +565,10 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       mbar_init(&bars->full[i], 1);
       mbar_init(&bars->empty[i], PIPE_CONS_WARPS);
     }
+    for (int i = 0; i < PIPE_TQ; i++) {
+      mbar_init(&bars->tq_full[i], 1);
+      mbar_init(&bars->tq_empty[i], PIPE_CONS_WARPS + PIPE_HALO_THREADS / 32);
+    }
     mbar_fence_init();
   }
   __syncthreads();
@@ -549,8 +584,15 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       if (lane == 0) {
         const uint64_t pol_once = policy_evict_first();
         RingPos rp = {0, 0u};
-        int k = 0;
-        for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+        int k = 0, kt = 0;
+        int tile = blockIdx.x;   // the host keeps gridDim.x <= ntiles
+        int tile_after = next_tile(g, a.sched, tile);
+        tq_push(bars, kt++, tile);
+        while (tile >= 0) {
+        // the halo warps run half a tile ahead of the arithmetic warps: they get the next index (or the end marker) now,
+        // and the draw for the tile after that is in flight while this tile is streamed
+        tq_push(bars, kt++, tile_after);
+        const int tile_after2 = tile_after >= 0 ? next_tile(g, a.sched, tile_after) : -1;
         for (int rhs = 0; rhs < nrhs; rhs++, k++) {   // all right-hand sides of a tile back to back: links and clover
                                                        // blocks of the 2nd..nth pass come out of L2
           if (k == 0) {
@@ -583,8 +625,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             rp.advance(nslot);
           }
           int next = tile, nr = rhs + 1;
-          if (nr == nrhs) { nr = 0; next = tile + gridDim.x; }
-          if (next < g.ntiles) {  // spinor of the next pass: its buffer is released after this pass's hops
+          if (nr == nrhs) { nr = 0; next = tile_after; }
+          if (next >= 0) {  // spinor of the next pass: its buffer is released after this pass's hops
             mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
@@ -592,12 +634,17 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
                        &bars->full_sp);
           }
         }
+        tile = tile_after;
+        tile_after = tile_after2;
+        }
       }
     } else {
       // ------------------------------ halo loaders: LDGSTS one stage ahead ----------------------------
       const int lt = tid - (PIPE_CONS_WARPS + 1) * 32;
       RingPos hp = {0, 0u};   // halo buffer ring
-      for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+      for (int kt = 0;; kt++) {
+      const int tile = tq_pop(bars, kt, lane);
+      if (tile < 0) break;
       for (int rhs = 0; rhs < nrhs; rhs++) {
         const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
         const T2<T>* in_r = a.in + rhs * a.rhs_stride;
@@ -607,6 +654,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           cp_async_arrive_noinc(&bars->full_h[hp.slot]);
           hp.advance(nhb);
         }
+      }
       }
     }
   } else {
@@ -624,7 +672,9 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     RingPos rp = {0, 0u};
     RingPos hp = {0, 0u};
     int k = 0;
-    for (int tile = blockIdx.x; tile < g.ntiles; tile += gridDim.x)
+    for (int kt = 0;; kt++) {
+    const int tile = tq_pop(bars, kt, lane);
+    if (tile < 0) break;
     for (int rhs = 0; rhs < nrhs; rhs++, k++) {
       const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
       const int x3 = __ldg(tab + 8) + l[3];
@@ -725,17 +775,31 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           for (int c = 0; c < 12; c++) nrm += (double)res[c].re * (double)res[c].re + (double)res[c].im * (double)res[c].im;
         }
       }
+      if (a.epi != EPI_STORE) {
+        // one partial sum per (right-hand side, tile), reduced in a fixed order: the result does not depend on which
+        // CTA happened to draw the tile.  s_red alternates between two rows, so one named barrier per pass is enough.
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+        if (lane == 0) s_red[k & 1][warp] = nrm;
+        asm volatile("bar.sync 1, %0;" ::"n"(PIPE_CONS_WARPS * 32) : "memory");
+        if (tid == 0) {
+          double s = 0;
+          for (int w = 0; w < PIPE_CONS_WARPS; w++) s += s_red[k & 1][w];
+          a.partial[(size_t)rhs * g.ntiles + tile] = s;
+        }
+        nrm = 0.0;
+      }
+    }
     }
   }
-  if (a.epi != EPI_STORE) {  // fixed-order CTA reduction over everything this CTA produced
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
-    if (lane == 0) s_red[warp] = nrm;
-    __syncthreads();
-    if (tid == 0) {
-      double s = 0;
-      for (int w = 0; w < PIPE_CONS_WARPS; w++) s += s_red[w];
-      a.partial[blockIdx.x] = s;
+  if (a.sched != nullptr) {   // the last CTA to finish puts the scheduler's counters back to zero for the next launch
+    if (tid == 0) {           // (thread 0 has seen the end-of-tiles marker, so this CTA's last draw is behind it)
+      __threadfence();
+      if (atomicAdd(a.sched + 1, 1u) == gridDim.x - 1) {
+        a.sched[0] = 0u;
+        a.sched[1] = 0u;
+        __threadfence();
+      }
     }
   }
 }
@@ -770,6 +834,15 @@ bool dw_set_mode(const char* name) {
 static int env_int(const char* name, int dflt) {
   const char* e = getenv(name);
   return e ? atoi(e) : dflt;
+}
+// LQCD_SCHED=static: tiles b, b + grid, ... per CTA instead of the global tile counter (an experiment switch)
+static bool pipe_dynamic() {
+  static int dyn = -1;
+  if (dyn < 0) {
+    const char* e = getenv("LQCD_SCHED");
+    dyn = (e && !strcmp(e, "static")) ? 0 : 1;
+  }
+  return dyn == 1;
 }
 // ---- host side: configuration of the persistent kernel ------------------------------------------------
 struct PipeCfg {
@@ -806,7 +879,12 @@ static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg&
   // than cache it in a process-wide variable that another device or thread would not see
   cudaError_t e = cudaFuncSetAttribute(dw_pipe_kernel<T, RECON, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
   if (e != cudaSuccess) return e;
-  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, a, c.nslot);
+  DwArgs<T> b = a;
+  static std::atomic<unsigned> launch_no(0);
+  // one pair of scheduler counters per launch in flight (a pool of SCHED_SLOTS pairs owned by the geometry, handed out
+  // round-robin): launches of the same geometry running concurrently on different streams do not share a counter
+  b.sched = (g.sched != nullptr && pipe_dynamic()) ? g.sched + 2 * (launch_no++ % SCHED_SLOTS) : nullptr;
+  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, b, c.nslot);
   count_launch();
   return cudaGetLastError();
 }
@@ -863,15 +941,15 @@ void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int 
   const PipeCfg pc = pipe_config<T>(g, recon, diag, parity);
   const char* tn = sizeof(T) == 8 ? "double" : "float";
   if (pc.use) {
-    snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=2 tile=%dx%dx%dx%d",
-             tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, g.b[0], g.b[1], g.b[2], g.b[3]);
+    snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=2 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
+             tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
     return;
   }
   const DirectCfg dc = direct_config<T>(g, recon, diag, parity);
-  snprintf(buf, (size_t)len, "%s<%s,%d,%d%s> grid=%d threads=%d smem=0 tile=%dx%dx%dx%d",
+  snprintf(buf, (size_t)len, "%s<%s,%d,%d%s> grid=%d threads=%d smem=0 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
            dc.kind == KIND_FULL ? "dw_kernel" : "dw_kernel_h", tn, recon, diag,
            dc.kind == KIND_FULL ? "" : (dc.kind == KIND_SPLIT ? ",split" : ",half"), dc.grid, dc.threads, g.b[0], g.b[1],
-           g.b[2], g.b[3]);
+           g.b[2], g.b[3], g.sw, g.c1, g.c2);
 }
 template void dw_describe<double>(const Geom&, int, int, int, char*, int);
 template void dw_describe<float>(const Geom&, int, int, int, char*, int);
@@ -879,7 +957,7 @@ template void dw_describe<float>(const Geom&, int, int, int, char*, int);
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity) {
   PipeCfg c = pipe_config<T>(g, recon, diag, parity);
-  return c.use ? c.grid : direct_config<T>(g, recon, diag, parity).grid;
+  return c.use ? g.ntiles : direct_config<T>(g, recon, diag, parity).grid;   // pipeline: one partial sum per tile
 }
 template int dw_num_partials<double>(const Geom&, int, int, int);
 template int dw_num_partials<float>(const Geom&, int, int, int);

@@ -26,6 +26,7 @@ struct DwArgs {
   int dagger;
   int parity;                          // -1: both parities; 0/1: only this output parity
   int epi;
+  unsigned int* sched;                 // pipeline kernel: {next tile, finished CTAs} of its tile scheduler (NULL: static)
   int nrhs;                            // > 1: in / out are arrays of nrhs spinor fields rhs_stride complex numbers apart
   long long rhs_stride;                //      (several right-hand sides share the links and the clover term)
 };

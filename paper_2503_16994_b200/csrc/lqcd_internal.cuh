@@ -9,9 +9,9 @@
 // (double2 / float2): component-major inside the tile so that the 32 lanes of a warp (consecutive j)
 // read 32 consecutive complex numbers = 512 B (fp64) / 256 B (fp32) per load instruction, and
 // tile-major outside so that one tile's data is one contiguous block of memory.
-// Tiles are ordered so that a linear sweep over the tile index walks the time direction inside a
-// chunk of (c1 x c2) tiles in (x2,x3): the working set between the first and last use of a spinor
-// or link then fits the 126 MB L2 (SURVEY.md section 7 "hard parts").
+// Tiles are ordered so that a linear sweep over the tile index walks one direction inside a chunk of
+// (c1 x c2) tiles in the other two of (x2,x3,x4): the working set between the first and last use of a
+// spinor or link then fits the 126 MB L2 (SURVEY.md section 7 "hard parts").
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -25,7 +25,8 @@ struct Geom {
   int b[4];       // tile extents (powers of two)
   int lb[4];      // log2: lb[0] = log2(b0/2), lb[1..3] = log2(b[1..3])
   int nt[4];      // tiles per direction
-  int c1, c2;     // L2 chunk, in tiles, along directions 1 and 2
+  int sw, da, db; // tile order: direction swept inside a chunk, and the two chunked directions (a permutation of 1,2,3)
+  int c1, c2;     // L2 chunk, in tiles, along directions da and db
   int TV;         // sites of one parity per tile
   int ntiles;
   int bc;         // lqcd_bc
@@ -34,28 +35,35 @@ struct Geom {
   // device table, TILE_TAB ints per tile: linear index of the 8 neighbour tiles (2*mu + (0: +mu, 1: -mu)),
   // then the time coordinate of the tile origin (library-owned, built by lqcd_geom_create)
   const int* tile_tab;
+  unsigned int* sched;   // SCHED_SLOTS pairs of counters for the pipeline kernel's tile scheduler (library-owned, zeroed)
   int sm_count;     // host-side launch configuration (SMs, opt-in shared memory per CTA)
   int smem_optin;
 };
-enum { TILE_TAB = 12 };
+enum { TILE_TAB = 12, SCHED_SLOTS = 64 };
 
-// ---- tile order: [T2hi][T1hi][T3][T2lo][T1lo][T0] -------------------------------------------------
+// ---- tile order: [Tb hi][Ta hi][Ts][Tb lo][Ta lo][T0] ----------------------------------------------
+// (sw, da, db) is a permutation of the directions (1, 2, 3): a linear sweep over the tile index walks direction sw
+// inside a chunk of c1 x c2 tiles along (da, db); direction 0 is always whole.  The faces cut by chunk borders are
+// those of da and db only -- the sweep direction's neighbours are one layer away -- so da and db are chosen among the
+// directions whose tile faces are contiguous runs in memory.
 __host__ __device__ inline int tile_linear(const Geom& g, int T0, int T1, int T2, int T3) {
-  int T1hi = T1 / g.c1, T1lo = T1 - T1hi * g.c1;
-  int T2hi = T2 / g.c2, T2lo = T2 - T2hi * g.c2;
-  int n1hi = g.nt[1] / g.c1;
-  return T0 + g.nt[0] * (T1lo + g.c1 * (T2lo + g.c2 * (T3 + g.nt[3] * (T1hi + n1hi * T2hi))));
+  const int T[4] = {T0, T1, T2, T3};
+  const int Ta = T[g.da], Tb = T[g.db], Ts = T[g.sw];
+  int Tahi = Ta / g.c1, Talo = Ta - Tahi * g.c1;
+  int Tbhi = Tb / g.c2, Tblo = Tb - Tbhi * g.c2;
+  int nahi = g.nt[g.da] / g.c1;
+  return T0 + g.nt[0] * (Talo + g.c1 * (Tblo + g.c2 * (Ts + g.nt[g.sw] * (Tahi + nahi * Tbhi))));
 }
 __host__ __device__ inline void tile_coords(const Geom& g, int t, int T[4]) {
-  int n1hi = g.nt[1] / g.c1;
+  int nahi = g.nt[g.da] / g.c1;
   T[0] = t % g.nt[0]; t /= g.nt[0];
-  int T1lo = t % g.c1; t /= g.c1;
-  int T2lo = t % g.c2; t /= g.c2;
-  T[3] = t % g.nt[3]; t /= g.nt[3];
-  int T1hi = t % n1hi; t /= n1hi;
-  int T2hi = t;
-  T[1] = T1hi * g.c1 + T1lo;
-  T[2] = T2hi * g.c2 + T2lo;
+  int Talo = t % g.c1; t /= g.c1;
+  int Tblo = t % g.c2; t /= g.c2;
+  T[g.sw] = t % g.nt[g.sw]; t /= g.nt[g.sw];
+  int Tahi = t % nahi; t /= nahi;
+  int Tbhi = t;
+  T[g.da] = Tahi * g.c1 + Talo;
+  T[g.db] = Tbhi * g.c2 + Tblo;
 }
 
 // local coordinates of checkerboard index j, parity p, inside a tile (tile origins are even)
