@@ -158,11 +158,20 @@ lqcd_status lqcd_spinor_dot(const lqcd_geom* g, const void* u, const void* v, in
 lqcd_status lqcd_correlator_ps(const lqcd_geom* g, const void* columns, int ncol, lqcd_prec prec, void* workspace,
                                double* C_host, void* stream);
 
-/* End-to-end convenience over HOST buffers in the canonical layout (allocates device scratch, copies in,
- * imports, builds the clover term if csw != 0, applies D or D^+, exports, copies back). */
+/* End-to-end call over HOST buffers in the canonical layout (SURVEY.md 8(b), 8(d) "e2e"; Csw! then
+ * Dw! on a configuration that lives on the host).  U_canon_host [V][4][3][3], in_canon_host / out_canon_host [V][4][3],
+ * complex fp64, HOST memory (pinned memory makes the copies asynchronous; pageable memory works).  The gauge field is
+ * copied in time slabs through two device staging buffers; each slab is converted to the internal layout and the
+ * clover term of the time slices whose neighbours have arrived is built while the next slab crosses PCIe; then the
+ * spinor is imported, D (dagger = 0) or D^+ applied in `prec`, the result exported and copied back.  The call returns
+ * when out_canon_host is valid.  Device scratch, streams and the geometry are kept by the library between calls and
+ * reused when desc, prec and recon are unchanged (one cached context per process, mutex-guarded);
+ * lqcd_host_cache_release() frees them.  Errors: LQCD_EINVAL (NULL, bad enum, kappa <= 0, LQCD_BC_SLAB),
+ * LQCD_ECUDA / LQCD_ENOMEM (the cache is released). */
 lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host,
                                const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
                                lqcd_recon recon);
+lqcd_status lqcd_host_cache_release(void);
 
 /* Time-direction domain decomposition (the volume one GPU holds
  * is the paper's stated limit).  A rank owns the slab x4 in [t0, t0 + L[3]) of a lattice periodic in time and creates
@@ -237,6 +246,9 @@ lqcd_status lqcd_dw_plan(const lqcd_geom* g, lqcd_prec prec, lqcd_recon recon, i
  * "pipe" (default: the warp-specialised shared-memory pipeline where the tile shape allows it), "stream"
  * (persistent one-thread-per-site CTAs), "split" (one parity of a tile per CTA), "direct" (one CTA per tile).
  * All four compute the same operator; the environment variable LQCD_DW_MODE sets the initial value.
+ * "host_slab": decimal string n >= 0, time slices per staged gauge slab of lqcd_dw_apply_host (0 = automatic: about
+ * 1/12 of the lattice, at least 64 MB).  "pipe_grid": decimal string n >= 0, at most n CTAs for the pipeline kernel (0 = default, one per SM) -- a test hook:
+ * with one or two CTAs each of them walks hundreds of tiles and wraps its mbarrier rings many times.
  * LQCD_EINVAL for an unknown key or value. */
 lqcd_status lqcd_set_option(const char* key, const char* value);
 

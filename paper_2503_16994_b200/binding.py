@@ -23,7 +23,7 @@ EXPORTS = [
     "lqcd_gauge_import", "lqcd_gauge_export", "lqcd_spinor_import", "lqcd_spinor_export",
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
-    "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
+    "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_host_cache_release", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
     "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
     "lqcd_clover_build_slab", "lqcd_cg_solve_slab",
 ]
@@ -308,6 +308,11 @@ def dw_apply_host(L, kappa, csw, U_canon, psi_canon, out_canon, bc=BC_PERIODIC, 
     d = _dirac(kappa, csw, ct, mu)
     _check(lib().lqcd_dw_apply_host(ctypes.byref(desc), ctypes.byref(d), _ptr(U_canon), _ptr(psi_canon), _ptr(out_canon),
                                     1 if dagger else 0, prec, recon))
+
+
+def host_cache_release():
+    """Free the device scratch lqcd_dw_apply_host keeps between calls."""
+    _check(lib().lqcd_host_cache_release())
 
 
 def dw_apply_multi(g, kappa, U, clover, src, dst, nrhs, prec=F64, recon=RECON_18, dagger=False, stream=None, mu=0.0):

@@ -8,6 +8,7 @@
 
 #include <atomic>
 #include <chrono>
+#include <mutex>
 #include <vector>
 
 #include "cg.cuh"
@@ -29,6 +30,12 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 void count_launch(int n) { g_launches += n; }
+
+// lqcd_set_option("host_slab", n): time slices per staged gauge slab of lqcd_dw_apply_host (0 = automatic); takes
+// effect when the cached host context is next rebuilt
+static int g_host_slab_opt = 0;
+static bool g_host_slab_changed = false;
+void set_host_slab(int n) { g_host_slab_changed = g_host_slab_changed || n != g_host_slab_opt; g_host_slab_opt = n; }
 
 static int ilog2(int v) {
   int l = 0;
@@ -217,6 +224,15 @@ lqcd_status lqcd_set_option(const char* key, const char* value) {
   REQUIRE(key && value, "lqcd_set_option: NULL argument");
   if (!strcmp(key, "dw_mode")) {
     REQUIRE(dw_set_mode(value), "lqcd_set_option: dw_mode must be pipe, stream, split or direct");
+    return LQCD_OK;
+  }
+  if (!strcmp(key, "host_slab")) {
+    REQUIRE(atoi(value) >= 0, "lqcd_set_option: host_slab must be >= 0");
+    lqcd::set_host_slab(atoi(value));
+    return LQCD_OK;
+  }
+  if (!strcmp(key, "pipe_grid")) {
+    REQUIRE(dw_set_pipe_grid(atoi(value)), "lqcd_set_option: pipe_grid must be >= 0");
     return LQCD_OK;
   }
   set_error("lqcd_set_option: unknown key '%s'", key);
@@ -971,66 +987,157 @@ lqcd_status lqcd_propagator(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_
   return LQCD_OK;
 }
 
-lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host, const void* in_canon_host,
-                               void* out_canon_host, int dagger, lqcd_prec prec, lqcd_recon recon) {
+}  // extern "C"
+// ---- host-buffer path -----------------------------------------------------------------------------------------
+// Device scratch, streams and the geometry of the last lqcd_dw_apply_host call are kept (one context per process,
+// guarded by a mutex) and reused when the next call has the same lattice, precision and link format: seven
+// cudaMalloc / cudaFree pairs and a geometry build per call otherwise cost tens of milliseconds.
+// lqcd_host_cache_release() frees them.
+namespace {
+struct HostCtx {
+  bool valid = false;
+  lqcd_geom_desc desc;
+  lqcd_prec prec;
+  lqcd_recon recon;
+  bool with_clover = false;
+  lqcd_geom* h = nullptr;
+  void *stage[2] = {nullptr, nullptr}, *dSc = nullptr, *dU64 = nullptr, *dU = nullptr, *dA = nullptr, *dIn = nullptr, *dOut = nullptr;
+  cudaStream_t s_copy = nullptr, s_comp = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_spinor = nullptr;
+  int slab = 0;   // time slices per staged chunk
+  void release() {
+    if (!valid && !h) return;
+    DeviceGuard dg(desc.device);
+    cudaDeviceSynchronize();
+    for (int i = 0; i < 2; i++) {
+      if (ev_copied[i]) cudaEventDestroy(ev_copied[i]);
+      if (ev_free[i]) cudaEventDestroy(ev_free[i]);
+      cudaFree(stage[i]);
+      ev_copied[i] = ev_free[i] = nullptr; stage[i] = nullptr;
+    }
+    if (ev_spinor) cudaEventDestroy(ev_spinor);
+    if (s_copy) cudaStreamDestroy(s_copy);
+    if (s_comp) cudaStreamDestroy(s_comp);
+    cudaFree(dSc); cudaFree(dU64); if (dU != dU64) cudaFree(dU); cudaFree(dA); cudaFree(dIn); cudaFree(dOut);
+    dSc = dU64 = dU = dA = dIn = dOut = nullptr;
+    ev_spinor = nullptr; s_copy = s_comp = nullptr;
+    lqcd_geom_destroy(h);
+    h = nullptr;
+    valid = false;
+  }
+};
+HostCtx g_host;
+std::mutex g_host_mutex;
+
+
+bool same_desc(const lqcd_geom_desc& a, const lqcd_geom_desc& b) {
+  bool same = a.bc == b.bc && a.device == b.device && a.slab_edges == b.slab_edges;
+  for (int i = 0; i < 4; i++) same = same && a.L[i] == b.L[i] && a.theta[i] == b.theta[i];
+  for (int i = 0; i < 3; i++) same = same && a.phi0[i] == b.phi0[i] && a.phiT[i] == b.phiT[i];
+  return same;
+}
+}  // namespace
+
+extern "C" lqcd_status lqcd_host_cache_release(void) {
+  std::lock_guard<std::mutex> lock(g_host_mutex);
+  g_host.release();
+  return LQCD_OK;
+}
+
+// The gauge field arrives in time slabs: while slab k + 1 crosses PCIe into one of two staging buffers, slab k is
+// converted to the internal layout and the clover term of every time slice whose neighbours are complete is built,
+// so that after the last byte of the field only one slab's import, two slices of Csw!, the operator, the export and
+// the copy back remain.  The spinor follows the gauge field on the copy stream (same PCIe direction).
+extern "C" lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd_dirac* d, const void* U_canon_host,
+                                          const void* in_canon_host, void* out_canon_host, int dagger, lqcd_prec prec,
+                                          lqcd_recon recon) {
   REQUIRE(desc && d && U_canon_host && in_canon_host && out_canon_host, "lqcd_dw_apply_host: NULL argument");
   REQUIRE(valid_prec(prec) && valid_recon(recon), "lqcd_dw_apply_host: bad precision / recon");
   REQUIRE(desc->bc != LQCD_BC_SLAB, "lqcd_dw_apply_host: a slab needs its neighbours' faces (lqcd_dw_slab_pack / _faces)");
-  lqcd_geom* h = nullptr;
-  lqcd_status st = lqcd_geom_create(desc, &h);
-  if (st != LQCD_OK) return st;
-  const size_t V = (size_t)2 * h->g.Vh;
-  const size_t gc = V * 36 * sizeof(double2), sc = V * 12 * sizeof(double2);
-  void *dUc = nullptr, *dSc = nullptr, *dU64 = nullptr, *dU = nullptr, *dA = nullptr, *dIn = nullptr, *dOut = nullptr;
-  cudaStream_t s1 = nullptr, s2 = nullptr;
-  cudaEvent_t ev_u = nullptr, ev_s = nullptr;
-  auto cleanup = [&]() {
-    cudaDeviceSynchronize();
-    if (ev_u) cudaEventDestroy(ev_u);
-    if (ev_s) cudaEventDestroy(ev_s);
-    if (s1) cudaStreamDestroy(s1);
-    if (s2) cudaStreamDestroy(s2);
-    cudaFree(dUc); cudaFree(dSc); cudaFree(dU64); if (dU != dU64) cudaFree(dU); cudaFree(dA); cudaFree(dIn); cudaFree(dOut);
-    lqcd_geom_destroy(h);
-  };
-#define HTRY(e, what) do { if (!cuda_ok((e), what)) { cleanup(); return LQCD_ECUDA; } } while (0)
-#define LTRY(e) do { lqcd_status _s = (e); if (_s != LQCD_OK) { cleanup(); return _s; } } while (0)
-  HTRY(cudaMalloc(&dUc, gc), "cudaMalloc");
-  HTRY(cudaMalloc(&dSc, sc), "cudaMalloc");
-  HTRY(cudaMalloc(&dU64, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F64, recon)), "cudaMalloc");
-  HTRY(cudaMalloc(&dIn, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
-  HTRY(cudaMalloc(&dOut, lqcd_field_bytes(h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
-  // two streams: the spinor's H2D copy (s2) runs while the gauge field is imported and the clover term built (s1);
-  // with pinned host buffers the copies are truly asynchronous, with pageable ones they are staged but still ordered
-  HTRY(cudaStreamCreate(&s1), "cudaStreamCreate");
-  HTRY(cudaStreamCreate(&s2), "cudaStreamCreate");
-  HTRY(cudaEventCreateWithFlags(&ev_u, cudaEventDisableTiming), "cudaEventCreate");
-  HTRY(cudaEventCreateWithFlags(&ev_s, cudaEventDisableTiming), "cudaEventCreate");
-  HTRY(cudaMemcpyAsync(dUc, U_canon_host, gc, cudaMemcpyHostToDevice, s1), "H2D gauge");
-  HTRY(cudaEventRecord(ev_u, s1), "event");
-  HTRY(cudaStreamWaitEvent(s2, ev_u, 0), "wait");   // same PCIe direction: the spinor follows the gauge field
-  HTRY(cudaMemcpyAsync(dSc, in_canon_host, sc, cudaMemcpyHostToDevice, s2), "H2D spinor");
-  LTRY(lqcd_spinor_import(h, dSc, dIn, prec, s2));
-  HTRY(cudaEventRecord(ev_s, s2), "event");
-  LTRY(lqcd_gauge_import(h, dUc, dU64, LQCD_F64, recon, s1));
-  if (d->csw != 0.0 || (desc->bc != LQCD_BC_PERIODIC && d->ct != 1.0)) {
-    HTRY(cudaMalloc(&dA, lqcd_field_bytes(h, LQCD_FIELD_CLOVER, prec, recon)), "cudaMalloc");
-    LTRY(lqcd_clover_build(h, d, dU64, recon, dA, nullptr, prec, s1));
+  REQUIRE(good_kappa(d), "lqcd_dw_apply_host: kappa must be positive and finite (got %g)", d->kappa);
+  std::lock_guard<std::mutex> lock(g_host_mutex);
+  HostCtx& c = g_host;
+  const bool with_clover = d->csw != 0.0 || (desc->bc != LQCD_BC_PERIODIC && d->ct != 1.0);
+#define HTRY(e, what) do { if (!cuda_ok((e), what)) { c.release(); return LQCD_ECUDA; } } while (0)
+#define LTRY(e) do { lqcd_status _s = (e); if (_s != LQCD_OK) { c.release(); return _s; } } while (0)
+  if (!(c.valid && !g_host_slab_changed && same_desc(c.desc, *desc) && c.prec == prec && c.recon == recon && c.with_clover == with_clover)) {
+    c.release();
+    lqcd_status st = lqcd_geom_create(desc, &c.h);
+    if (st != LQCD_OK) return st;
+    c.desc = *desc; c.prec = prec; c.recon = recon; c.with_clover = with_clover;
+    DeviceGuard dg(desc->device);
+    const Geom& g = c.h->g;
+    const size_t V3 = (size_t)g.L[0] * g.L[1] * g.L[2];
+    // slab: a whole number of slices, about 1/12 of the field but not below 64 MB (a copy that short does not reach
+    // the link's bandwidth) and not more than the lattice
+    int slab = (g.L[3] + 11) / 12;
+    while ((size_t)slab * V3 * 36 * sizeof(double2) < ((size_t)64 << 20) && slab < g.L[3]) slab++;
+    if (g_host_slab_opt > 0) slab = g_host_slab_opt < g.L[3] ? g_host_slab_opt : g.L[3];   // lqcd_set_option("host_slab")
+    g_host_slab_changed = false;
+    c.slab = slab;
+    HTRY(cudaMalloc(&c.stage[0], (size_t)slab * V3 * 36 * sizeof(double2)), "cudaMalloc");
+    HTRY(cudaMalloc(&c.stage[1], (size_t)slab * V3 * 36 * sizeof(double2)), "cudaMalloc");
+    HTRY(cudaMalloc(&c.dSc, (size_t)2 * g.Vh * 12 * sizeof(double2)), "cudaMalloc");
+    HTRY(cudaMalloc(&c.dU64, lqcd_field_bytes(c.h, LQCD_FIELD_GAUGE, LQCD_F64, recon)), "cudaMalloc");
+    if (prec == LQCD_F64) c.dU = c.dU64;
+    else HTRY(cudaMalloc(&c.dU, lqcd_field_bytes(c.h, LQCD_FIELD_GAUGE, LQCD_F32, recon)), "cudaMalloc");
+    if (with_clover) HTRY(cudaMalloc(&c.dA, lqcd_field_bytes(c.h, LQCD_FIELD_CLOVER, prec, recon)), "cudaMalloc");
+    HTRY(cudaMalloc(&c.dIn, lqcd_field_bytes(c.h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
+    HTRY(cudaMalloc(&c.dOut, lqcd_field_bytes(c.h, LQCD_FIELD_SPINOR, prec, recon)), "cudaMalloc");
+    HTRY(cudaStreamCreate(&c.s_copy), "cudaStreamCreate");
+    HTRY(cudaStreamCreate(&c.s_comp), "cudaStreamCreate");
+    for (int i = 0; i < 2; i++) {
+      HTRY(cudaEventCreateWithFlags(&c.ev_copied[i], cudaEventDisableTiming), "cudaEventCreate");
+      HTRY(cudaEventCreateWithFlags(&c.ev_free[i], cudaEventDisableTiming), "cudaEventCreate");
+    }
+    HTRY(cudaEventCreateWithFlags(&c.ev_spinor, cudaEventDisableTiming), "cudaEventCreate");
+    c.valid = true;
   }
-  if (prec == LQCD_F64) dU = dU64;
-  else {
-    HTRY(cudaMalloc(&dU, lqcd_field_bytes(h, LQCD_FIELD_GAUGE, LQCD_F32, recon)), "cudaMalloc");
-    LTRY(lqcd_gauge_import(h, dUc, dU, LQCD_F32, recon, s1));
+  DeviceGuard dg(desc->device);
+  const lqcd_geom* h = c.h;
+  const Geom& g = h->g;
+  const size_t V3 = (size_t)g.L[0] * g.L[1] * g.L[2];
+  const size_t slice_bytes = V3 * 36 * sizeof(double2);
+  const size_t sc = (size_t)2 * g.Vh * 12 * sizeof(double2);
+  CloverParm cp;
+  cp.kappa = d->kappa; cp.csw = d->csw; cp.ct = d->ct;
+  for (int i = 0; i < 3; i++) cp.phiT[i] = desc->phiT[i];
+  int built = 1;   // slices [1, built) of the clover term are done (slice 0 needs the last slice: at the end)
+  int k = 0;
+  for (int t0 = 0; t0 < g.L[3]; t0 += c.slab, k++) {
+    const int t1 = t0 + c.slab < g.L[3] ? t0 + c.slab : g.L[3];
+    const int b = k & 1;
+    if (k >= 2) HTRY(cudaStreamWaitEvent(c.s_copy, c.ev_free[b], 0), "wait");
+    HTRY(cudaMemcpyAsync(c.stage[b], (const char*)U_canon_host + (size_t)t0 * slice_bytes, (size_t)(t1 - t0) * slice_bytes,
+                         cudaMemcpyHostToDevice, c.s_copy), "H2D gauge slab");
+    HTRY(cudaEventRecord(c.ev_copied[b], c.s_copy), "event");
+    HTRY(cudaStreamWaitEvent(c.s_comp, c.ev_copied[b], 0), "wait");
+    HTRY(gauge_import_slab<double>(g, c.stage[b], c.dU64, (int)recon, t0, t1, c.s_comp), "gauge_import (slab)");
+    if (prec == LQCD_F32) HTRY(gauge_import_slab<float>(g, c.stage[b], c.dU, (int)recon, t0, t1, c.s_comp), "gauge_import (slab)");
+    HTRY(cudaEventRecord(c.ev_free[b], c.s_comp), "event");
+    if (with_clover && t1 - 1 > built) {   // slices below t1 - 1 have both time neighbours on the device
+      cp.t_lo = built; cp.t_hi = t1 - 1;
+      HTRY(clover_build(g, cp, c.dU64, (int)recon, c.dA, nullptr, (int)prec, c.s_comp), "clover_build (slab)");
+      built = t1 - 1;
+    }
   }
-  HTRY(cudaStreamWaitEvent(s1, ev_s, 0), "wait");
-  LTRY(dw_common(h, d, dU, dA, dIn, dOut, prec, recon, s1, dagger != 0));
-  LTRY(lqcd_spinor_export(h, dOut, dSc, prec, s1));
-  HTRY(cudaMemcpyAsync(out_canon_host, dSc, sc, cudaMemcpyDeviceToHost, s1), "D2H spinor");
-  HTRY(cudaStreamSynchronize(s1), "sync");
-  cleanup();
+  HTRY(cudaMemcpyAsync(c.dSc, in_canon_host, sc, cudaMemcpyHostToDevice, c.s_copy), "H2D spinor");
+  HTRY(cudaEventRecord(c.ev_spinor, c.s_copy), "event");
+  if (with_clover) {
+    cp.t_lo = built; cp.t_hi = g.L[3];
+    HTRY(clover_build(g, cp, c.dU64, (int)recon, c.dA, nullptr, (int)prec, c.s_comp), "clover_build (last slices)");
+    cp.t_lo = 0; cp.t_hi = 1;
+    HTRY(clover_build(g, cp, c.dU64, (int)recon, c.dA, nullptr, (int)prec, c.s_comp), "clover_build (slice 0)");
+  }
+  HTRY(cudaStreamWaitEvent(c.s_comp, c.ev_spinor, 0), "wait");
+  LTRY(lqcd_spinor_import(h, c.dSc, c.dIn, prec, c.s_comp));
+  LTRY(dw_common(h, d, c.dU, with_clover ? c.dA : nullptr, c.dIn, c.dOut, prec, recon, c.s_comp, dagger != 0));
+  LTRY(lqcd_spinor_export(h, c.dOut, c.dSc, prec, c.s_comp));
+  HTRY(cudaMemcpyAsync(out_canon_host, c.dSc, sc, cudaMemcpyDeviceToHost, c.s_comp), "D2H spinor");
+  HTRY(cudaStreamSynchronize(c.s_comp), "sync");
+  HTRY(cudaStreamSynchronize(c.s_copy), "sync");
 #undef HTRY
 #undef LTRY
   return LQCD_OK;
 }
 
-}  // extern "C"

@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(CLV_THREADS, CLV_MINB) clover_kernel(const Clo
   local_coords(g, j, p, sp.l);
   sp.x3 = __ldg(g.tile_tab + (size_t)tile * TILE_TAB + 8) + sp.l[3];
   const int x3 = sp.x3;
+  if (x3 < cp.t_lo || x3 >= cp.t_hi) return;   // no barrier in this kernel: threads may leave on their own
 
   const bool fz = (g.bc != LQCD_BC_PERIODIC) && frozen_slice(g, x3);
   const double cc = cp.kappa * cp.csw;

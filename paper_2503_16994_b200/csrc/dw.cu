@@ -825,6 +825,14 @@ static int dw_mode() {
   }
   return g_mode;
 }
+// lqcd_set_option("pipe_grid", n): at most n CTAs for the pipeline kernel (0 = one per SM).  A test hook: with one or
+// two CTAs every CTA walks hundreds of tiles, i.e. every slot and phase of its mbarrier rings many times over.
+static int g_pipe_grid = 0;
+bool dw_set_pipe_grid(int n) {
+  if (n < 0) return false;
+  g_pipe_grid = n;
+  return true;
+}
 bool dw_set_mode(const char* name) {
   const int m = mode_from_name(name);
   if (m < 0) return false;
@@ -869,6 +877,7 @@ static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
   c.nslot = nslot;
   c.smem = sp + (size_t)nslot * slot + halo + sizeof(PipeBars);
   c.grid = g.sm_count;
+  if (g_pipe_grid > 0 && g_pipe_grid < c.grid) c.grid = g_pipe_grid;
   if (c.grid > g.ntiles) c.grid = g.ntiles;
   return c;
 }

@@ -39,6 +39,7 @@ int dw_num_partials(const Geom& g, int recon, int diag, int parity);
 template <typename T>
 void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int len);
 bool dw_set_mode(const char* name);
+bool dw_set_pipe_grid(int n);
 
 template <typename T>
 cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cudaStream_t s);

@@ -6,6 +6,8 @@ namespace lqcd {
 
 // layout.cu
 template <typename T> cudaError_t gauge_import(const Geom& g, const void* canon, void* U, int recon, cudaStream_t s);
+// the time slab t_lo <= x4 < t_hi only; canon_slab points at the first site of slice t_lo
+template <typename T> cudaError_t gauge_import_slab(const Geom& g, const void* canon_slab, void* U, int recon, int t_lo, int t_hi, cudaStream_t s);
 template <typename T> cudaError_t gauge_export(const Geom& g, const void* U, void* canon, int recon, cudaStream_t s);
 template <typename T> cudaError_t spinor_import(const Geom& g, const void* canon, void* psi, cudaStream_t s);
 template <typename T> cudaError_t spinor_export(const Geom& g, const void* psi, void* canon, cudaStream_t s);
@@ -17,6 +19,7 @@ cudaError_t to_f32(const void* src, void* dst, size_t ncomplex, cudaStream_t s);
 struct CloverParm {
   double kappa, csw, ct;
   double phiT[3];
+  int t_lo = 0, t_hi = 1 << 30;   // only sites with t_lo <= x4 < t_hi are built (the host path builds time slabs as they arrive)
 };
 // halo_lo / halo_hi: LQCD_BC_SLAB only (the neighbour ranks' adjacent time slices, canonical fp64 layout)
 cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, int recon, void* clover, void* clover_inv,

@@ -26,9 +26,12 @@ __device__ __forceinline__ bool site_from_thread(const Geom& g, SiteId& s) {
 }
 
 template <typename T>
-__global__ void gauge_import_kernel(const Geom g, const double2* __restrict__ canon, typename vec2<T>::type* U, int recon) {
+__global__ void gauge_import_kernel(const Geom g, const double2* __restrict__ canon, typename vec2<T>::type* U, int recon,
+                                    const int t_lo, const int t_hi) {
   SiteId s;
   if (!site_from_thread(g, s)) return;
+  if (s.x[3] < t_lo || s.x[3] >= t_hi) return;
+  s.n -= (long long)t_lo * g.L[0] * g.L[1] * g.L[2];   // canon starts at slice t_lo
   const int NCU = recon == 12 ? 6 : 9;
   for (int mu = 0; mu < 4; mu++)
     for (int c = 0; c < NCU; c++) {
@@ -125,7 +128,13 @@ static inline unsigned site_blocks(const Geom& g) { return (unsigned)((2 * g.Vh 
 
 template <typename T>
 cudaError_t gauge_import(const Geom& g, const void* canon, void* U, int recon, cudaStream_t s) {
-  gauge_import_kernel<T><<<site_blocks(g), 256, 0, s>>>(g, (const double2*)canon, (typename vec2<T>::type*)U, recon);
+  gauge_import_kernel<T><<<site_blocks(g), 256, 0, s>>>(g, (const double2*)canon, (typename vec2<T>::type*)U, recon, 0, g.L[3]);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T>
+cudaError_t gauge_import_slab(const Geom& g, const void* canon_slab, void* U, int recon, int t_lo, int t_hi, cudaStream_t s) {
+  gauge_import_kernel<T><<<site_blocks(g), 256, 0, s>>>(g, (const double2*)canon_slab, (typename vec2<T>::type*)U, recon, t_lo, t_hi);
   count_launch();
   return cudaGetLastError();
 }
@@ -174,6 +183,7 @@ cudaError_t point_source(const Geom& g, const int y[4], int spin, int colour, vo
 
 #define INST(T)                                                                                  \
   template cudaError_t gauge_import<T>(const Geom&, const void*, void*, int, cudaStream_t);      \
+  template cudaError_t gauge_import_slab<T>(const Geom&, const void*, void*, int, int, int, cudaStream_t); \
   template cudaError_t gauge_export<T>(const Geom&, const void*, void*, int, cudaStream_t);      \
   template cudaError_t spinor_import<T>(const Geom&, const void*, void*, cudaStream_t);          \
   template cudaError_t spinor_export<T>(const Geom&, const void*, void*, cudaStream_t);          \

@@ -153,6 +153,7 @@ template <typename T> __device__ __forceinline__ void st(typename vec2<T>::type*
 void set_error(const char* fmt, ...);
 bool cuda_ok(cudaError_t e, const char* what);
 void count_launch(int n = 1);
+void set_host_slab(int n);
 
 }  // namespace lqcd
 

@@ -257,3 +257,32 @@ def test_blas_reductions():
         # run-to-run bit reproducibility (fixed-order reduction)
         assert B.spinor_norm2(lat.g, da, ws, prec=prec) == n2
     lat.close()
+
+
+@pytest.mark.parametrize("L,bc,theta,phiT", [c for c in CASES if c[0] != (2, 2, 2, 2)])
+@pytest.mark.parametrize("slab", [0, 1, 3])
+def test_dw_apply_host_time_slabs(L, bc, theta, phiT, slab):
+    """The host path stages the gauge field in time slabs and builds the clover term slab by slab as the neighbours
+    arrive (slab = 3 leaves a ragged last slab; 1 = slice by slice; 0 = automatic, one slab on these small lattices):
+    same result as the oracle for every boundary condition; the cached context is reused by the second call and
+    rebuilt when the lattice or the slab size changes."""
+    kappa, csw, ct = 0.1355, 1.8, (1.0 if bc == B.BC_PERIODIC else 1.15)
+    U, psi = make_inputs(L, bc, 171)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc, phiT=phiT, ct=ct)
+    mask = interior(L, bc)
+    B.set_option("host_slab", str(slab))
+    try:
+        for rep, (prec, recon) in enumerate(((B.F64, B.RECON_18), (B.F64, B.RECON_18), (B.F32, B.RECON_12))):
+            for dagger in (False, True):
+                out = np.full_like(psi, np.nan)
+                B.dw_apply_host(L, kappa, csw, U, psi, out, bc=bc, theta=theta, phi0=synth.SF_PHI0, phiT=phiT,
+                                dagger=dagger, prec=prec, recon=recon, ct=ct)
+                if prec == B.F64:
+                    ref = oracle.dw(L, U, psi, kappa, A, bc=bc, theta=theta, dagger=dagger)
+                else:
+                    ref = oracle.dw(L, round_f32(U), round_f32(psi), kappa, round_f32(A), bc=bc, theta=theta, dagger=dagger)
+                assert site_rel_err(out, ref, mask) <= TOL[prec]
+                assert np.all(out[~mask] == 0)
+    finally:
+        B.set_option("host_slab", "0")
+        B.host_cache_release()

@@ -205,3 +205,74 @@ def test_cg_source_on_frozen_slice_is_ignored(eo):
                       clover_inv64=lat.Ainv[B.F64], eo=eo)
     assert info["iters"] == 0 and torch.count_nonzero(x).item() == 0
     lat.close()
+
+
+@pytest.mark.parametrize("grid", [1, 2, 5])
+@pytest.mark.parametrize("prec,recon", [(B.F64, B.RECON_18), (B.F32, B.RECON_12)])
+def test_pipeline_rings_many_wraps(grid, prec, recon):
+    """compute-sanitizer is closed on this GPU pool, so the hand-rolled mbarrier rings of dw_pipe_kernel (stage ring,
+    halo ring, spinor buffer, tile queue) are stressed instead: with 1, 2 or 5 CTAs for 128 tiles each CTA walks up to
+    128 tiles -- 1024 ring stages, every slot and both phase parities hundreds of times, the tile counter drawn 127
+    times -- and the result must still be the oracle's, for D and D^+ and through the fused CG epilogues."""
+    L, bc, theta, kappa, csw = (16, 8, 8, 16), B.BC_OPEN, (0.5, 0.5, 0.5, 0.0), 0.137, 1.9
+    U, psi = inputs(L, bc, 71)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
+    Uo, psio, Ao = (round_f32(U), round_f32(psi), round_f32(A)) if prec == B.F32 else (U, psi, A)
+    lat = Lattice(L, bc, theta)
+    lat.set_gauge(U, recons=(recon,), precs=(prec,))
+    lat.build_clover(kappa, csw, recon=recon, precs=(prec,))
+    assert B.geom_info(lat.g)[1] == [4, 2, 2, 4]
+    B.set_option("pipe_grid", str(grid))
+    try:
+        assert "grid=%d " % grid in B.dw_plan(lat.g, prec, recon, True)
+        mask = interior(L, bc)
+        for dagger in (False, True):
+            ref = oracle.dw(L, Uo, psio, kappa, Ao, bc=bc, theta=theta, dagger=dagger)
+            for rep in range(2):   # twice: the self-resetting tile counter must be back at zero
+                got = lat.dw(kappa, psi, prec, recon, dagger)
+                assert site_rel_err(got, ref, mask) <= TOL[prec]
+                assert np.all(got[~mask] == 0)
+        if prec == B.F64:
+            b = synth.point_source(L, (3, 2, 1, 8), 1, 1)
+            xo, it_o, _, _ = oracle.cg(L, U, b, kappa, A, bc=bc, theta=theta, tol=1e-9, maxiter=400)
+            x, ws = lat.alloc(B.FIELD_SPINOR), lat.alloc(B.FIELD_WORKSPACE)
+            info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, recon)], lat.A[B.F64], lat.spinor(b), x, ws, tol=1e-9,
+                              maxiter=400, recon=recon, raise_on_notconv=False)
+            assert abs(info["iters"] - abs(it_o)) <= 2
+    finally:
+        B.set_option("pipe_grid", "0")
+    lat.close()
+
+
+@pytest.mark.parametrize("mode", MODES, indirect=True)
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_no_write_outside_the_output(mode, prec):
+    """Out-of-bounds evidence without a sanitizer: every field lives inside one allocation between poisoned guard
+    bands; after D, D^+ and a CG solve in each kernel variant the guards and all the INPUT fields are bit-unchanged."""
+    L, kappa, csw = (8, 8, 4, 8), 0.13, 1.5
+    U, psi = inputs(L, B.BC_PERIODIC, 75)
+    lat = Lattice(L)
+    lat.set_gauge(U, precs=(prec,))
+    lat.build_clover(kappa, csw, precs=(prec,))
+    G = 1 << 16   # guard bytes on both sides
+    nb = B.field_bytes(lat.g, B.FIELD_SPINOR, prec)
+    def guarded(n):
+        buf = torch.full((n + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+        return buf, buf[G:G + n]
+    src_all, src = guarded(nb)
+    dst_all, dst = guarded(nb)
+    src.copy_(lat.spinor(psi, prec))
+    Ucopy, Acopy, src_copy = lat.U[(prec, 18)].clone(), lat.A[prec].clone(), src_all.clone()
+    for fn in (B.dw_apply, B.dwdag_apply):
+        fn(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src, dst, prec, 18)
+    if prec == B.F64:
+        ws_n = B.field_bytes(lat.g, B.FIELD_WORKSPACE)
+        ws_all, ws = guarded(ws_n)
+        B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, dst, ws, tol=1e-8, maxiter=50, raise_on_notconv=False)
+        torch.cuda.synchronize()
+        assert torch.all(ws_all[:G] == 0xA5) and torch.all(ws_all[G + ws_n:] == 0xA5)
+    torch.cuda.synchronize()
+    assert torch.all(dst_all[:G] == 0xA5) and torch.all(dst_all[G + nb:] == 0xA5)
+    assert torch.equal(src_all, src_copy)
+    assert torch.equal(lat.U[(prec, 18)], Ucopy) and torch.equal(lat.A[prec], Acopy)
+    lat.close()
