@@ -251,6 +251,18 @@ def run_ours(args):
     ms_local = e0.elapsed_time(e1)
     clocks = sampler.result()
     barrier()
+    # SURVEY.md 8(d) "Timing": the same K-step batch five more times, median and min reported beside the headline
+    # (which stays the first batch, the one the clock sampler and the launch counter bracket)
+    reps = []
+    for _ in range(5):
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        for _ in range(args.steps):
+            step()
+        r1.record()
+        torch.cuda.synchronize()
+        reps.append(r0.elapsed_time(r1) / args.steps)
+    reps_sorted = sorted(reps)
     ms = max_over_ranks(torch, dist, ms_local, "cuda")
     ms_per_step = ms / args.steps
     flops_step = 2.0 * FLOP_DW * V
@@ -268,7 +280,9 @@ def run_ours(args):
                 "frac_of_nominal_8TBs": round(achieved / NOMINAL_HBM_GBS, 4),
                 "bytes_per_launch": bytes_launch, "ms_per_launch": round(ms_launch, 4),
                 "model": "%d reals/site compulsory (links + psi in + psi out + clover), each datum once" % REALS_DW[recon],
-                "traffic": NCU_TRAFFIC.get((args.lattice, args.prec, recon))}
+                "repeats_ms_per_step": {"batches": [round(r, 4) for r in reps], "median": round(reps_sorted[2], 4),
+                                        "min": round(reps_sorted[0], 4)}}
+    roofline.update(ncu_traffic(args.lattice, args.prec, recon, plan))
 
     # e2e: same metric through the host-buffer C-ABI call, H2D and D2H inside the timed region
     e2e = None
@@ -298,10 +312,29 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the stencil kernel from the committed ncu --set full
-# capture (profiles/r01_v3_dw_pipe_kernel_f64_full.txt); keyed by (lattice, prec, recon).  None = not captured for
-# that configuration.
-NCU_TRAFFIC = {("48x48x48x96", "f64", 18): 17142972000 + 2026305000}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the stencil kernel, copied from the committed ncu --set full
+# capture named beside it; keyed by (lattice, prec, recon).  A capture belongs to one kernel configuration: `plan` is
+# the launch description (lqcd_dw_plan) the capture was taken with, and the number is dropped (null) when the
+# running library describes its launch differently, i.e. when the kernel or its tiling changed since the capture.
+NCU_TRAFFIC = {
+    ("48x48x48x96", "f64", 18): {
+        "bytes": 15717323000 + 2025048000,
+        "capture": "profiles/r02_dw_pipe_kernel_f64_full.txt",
+        "plan": "dw_pipe_kernel<double,18,1> grid=148 threads=384 smem=227648 ring_slots=3 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
+    ("48x48x48x96", "f32", 18): {
+        "bytes": 8046293000 + 1009103000,
+        "capture": "profiles/r02_dw_pipe_kernel_f32_full.txt",
+        "plan": "dw_pipe_kernel<float,18,1> grid=148 threads=384 smem=132416 ring_slots=4 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
+}
+
+
+def ncu_traffic(lattice, prec, recon, plan):
+    e = NCU_TRAFFIC.get((lattice, prec, recon))
+    if e is None:
+        return {"traffic": None, "traffic_source": "no ncu capture for this configuration"}
+    if e["plan"] != plan:
+        return {"traffic": None, "traffic_source": "stale: %s was captured with launch '%s'" % (e["capture"], e["plan"])}
+    return {"traffic": e["bytes"], "traffic_source": e["capture"]}
 
 
 def run_e2e(torch, B, S, args, L, prec, recon, dist):
