@@ -375,7 +375,7 @@ enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX
        PIPE_TQ = 4 };
 struct PipeBars {
   uint64_t full_sp, empty_sp;
-  uint64_t full_h[2], empty_h[2];
+  uint64_t full_h[4], empty_h[4];   // two halo buffers (full lattice), three (half lattice)
   uint64_t full[PIPE_MAX_SLOTS], empty[PIPE_MAX_SLOTS];
   uint64_t tq_full[PIPE_TQ], tq_empty[PIPE_TQ];   // tile queue: the producer lane tells the other warps which tile is next
   int tq[PIPE_TQ];
@@ -737,6 +737,10 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           }
         }
       }
+      // (pipe.cuh: release_fence.  The ring and halo releases above go without it: their refills come from DRAM / L2 a
+      // microsecond after the arrive, and every value loaded from a slot feeds the stage's own arithmetic; a fence per
+      // stage costs 1.2 % at 48^3 x 96.)
+      release_fence();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->empty_sp);   // spinor tile no longer needed: next tile's may land
       if (DIAG == DIAG_PRE) {
@@ -794,6 +798,342 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   }
   if (a.sched != nullptr) {   // the last CTA to finish puts the scheduler's counters back to zero for the next launch
     if (tid == 0) {           // (thread 0 has seen the end-of-tiles marker, so this CTA's last draw is behind it)
+      __threadfence();
+      if (atomicAdd(a.sched + 1, 1u) == gridDim.x - 1) {
+        a.sched[0] = 0u;
+        a.sched[1] = 0u;
+        __threadfence();
+      }
+    }
+  }
+}
+
+// =====================================================================================================
+// Half-lattice version of the pipeline kernel (output parity P = a.parity): the two passes of the even-odd operator
+// (D8:  tmp_o = A_oo^-1 H_oe in_e  [DIAG_POST],   out_e = A_ee in_e - kappa^2 H_eo tmp_o  [DIAG_PRE]).
+// A tile has only 128 output sites, so the eight arithmetic warps split the WORK of a site instead of the sites:
+//   * hops: warps 0-3 ("group F") take the forward hop of every direction, warps 4-7 ("group B") the backward hop of
+//     the same site -- disjoint operands (U_mu(x), psi(x+mu) against U_mu(x-mu), psi(x-mu)), twelve accumulators each;
+//   * after the last hop the groups swap halves through the (then dead) input-spinor buffer: F ends up with the
+//     complete upper chirality (components 0-5), B with the lower one (6-11);
+//   * the packed 6x6 blocks are block-diagonal in chirality: F multiplies with A+ (clover stages 0, 1), B with A-
+//     (stages 2, 3), and each group writes its six components.  No further exchange.
+// Stage order L0 L1 L2 L3 C C C C (DIAG_POST needs the complete hop sum before the block multiply); three halo buffers of
+// 32 columns (only the input parity's face sites are needed) give every halo two stages of lead.  Per tile the kernel
+// streams both parities of the links (all of them are used: forward hops take the links of the output parity, backward
+// hops those of the input parity), one parity of the input spinor, of the self spinor (DIAG_PRE) and of the blocks.
+// =====================================================================================================
+enum { HALF_NHB = 3, HALF_NF = 32, HALF_HS = HALF_NHB * HALF_NF, HALF_CLV_ROWS = 9 };
+
+template <typename T, int NCU>
+__device__ __forceinline__ void halo_load_half(const Geom& g, const DwArgs<T>& a, const int* __restrict__ tab, const int mu,
+                                               const int q, T2<T>* hb, const int lt) {
+  constexpr int TV = PIPE_TV;
+  const int tf = __ldg(tab + 2 * mu), tb = __ldg(tab + 2 * mu + 1);
+  for (int u = lt; u < 3 * HALF_NF; u += PIPE_HALO_THREADS) {
+    const int kind = u / HALF_NF;      // 0: F, 1: B, 2: BU
+    const int f = u - kind * HALF_NF;  // face index of the parity-q site
+    const int jn = face_site(mu, q, f, kind == 0 ? 0 : 3);
+    if (kind < 2) {
+      const T2<T>* src = a.in + field_offset(g, 12, q, kind == 0 ? tf : tb, 0, jn);
+      T2<T>* dst = hb + kind * 12 * HALF_HS + f;
+#pragma unroll
+      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * HALF_HS, src + c * TV);
+    } else {
+      const T2<T>* src = a.U + field_offset(g, 4 * NCU, q, tb, mu * NCU, jn);
+      T2<T>* dst = hb + 24 * HALF_HS + f;
+#pragma unroll
+      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * HALF_HS, src + c * TV);
+    }
+  }
+}
+
+// one hop of direction MU for one output site: FWD (group F) or backward (group B)
+template <typename T, int RECON, int MU, bool FWD>
+__device__ __forceinline__ void hop_one(const Geom& g, const DwArgs<T>& a, const T2<T>* sp_in, const T2<T>* ub, const T2<T>* hb,
+                                        const int p, const int j, const int (&l)[4], const int x3, const bool nonper, const T sg,
+                                        cx<T> (&acc)[12]) {
+  constexpr int NCU = (RECON == 12) ? 6 : 9;
+  constexpr int TV = PIPE_TV;
+  const int q = 1 - p;
+  const int l0h = l[0] >> 1;
+  const int fidx = face_index<MU>(l);
+  constexpr int stride = MU == 1 ? 2 : (MU == 2 ? 8 : 32);
+  if (MU == 3 && nonper && time_hop_blocked(g, x3, FWD)) return;
+  if (FWD) {
+    const bool cr = (l[MU] == 3);
+    int jn;
+    if (MU == 0) jn = j - l0h + ((l[0] + 1) >> 1);
+    else jn = j + stride;
+    const T2<T>* ps = cr ? hb + fidx : sp_in + jn;
+    hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, cr ? (int)HALF_HS : TV, TV, sg, a.has_theta, a.theta[MU], acc);
+  } else {
+    const bool cr = (l[MU] == 0);
+    int jn;
+    if (MU == 0) jn = j - l0h + ((l[0] - 1) >> 1);
+    else jn = j - stride;
+    const T2<T>* ps = cr ? hb + 12 * HALF_HS + fidx : sp_in + jn;
+    const T2<T>* us = cr ? hb + 24 * HALF_HS + fidx : ub + (q * NCU) * TV + jn;
+    hop_dir<T, RECON, MU, false, false>(ps, us, cr ? (int)HALF_HS : TV, cr ? (int)HALF_HS : TV, -sg, a.has_theta, a.theta[MU], acc);
+  }
+}
+
+template <typename T, int RECON, int DIAG>
+__global__ void __launch_bounds__(PIPE_THREADS, 1)
+dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
+  constexpr int NCU = (RECON == 12) ? 6 : 9;
+  constexpr int NSTC = (DIAG == DIAG_ONE) ? 0 : 4;          // block stages per tile: two per chirality, 9 rows each
+  constexpr bool SELF = (DIAG != DIAG_POST);                // the self spinor is staged too
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ double s_red[2][PIPE_CONS_WARPS];
+  if (a.skip != nullptr && *a.skip != 0) return;  // CG finished: uniform early exit
+  constexpr int TV = PIPE_TV;
+  const int tid = threadIdx.x;
+  const int lane = tid & 31;
+  const int warp = tid >> 5;
+  const int p = a.parity, q = 1 - p;
+  T2<T>* sp_in = reinterpret_cast<T2<T>*>(smem_raw);        // [12][TV] input spinor, parity q; exchange area after the hops
+  T2<T>* sp_self = sp_in + 12 * TV;                         // [12][TV] self spinor, parity p (SELF)
+  T2<T>* ring = sp_self + (SELF ? 12 * TV : 0);             // nslot x [2][NCU][TV] (block stages use the first 9 rows)
+  T2<T>* halo = ring + nslot * 2 * NCU * TV;                // [24 + NCU][HALF_HS]: three halo buffers of 32 columns
+  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * HALF_HS);
+  if (tid == 0) {
+    mbar_init(&bars->full_sp, 1);
+    mbar_init(&bars->empty_sp, PIPE_CONS_WARPS);
+    for (int i = 0; i < HALF_NHB; i++) {
+      mbar_init(&bars->full_h[i], PIPE_HALO_THREADS);
+      mbar_init(&bars->empty_h[i], PIPE_CONS_WARPS);
+    }
+    for (int i = 0; i < nslot; i++) {
+      mbar_init(&bars->full[i], 1);
+      mbar_init(&bars->empty[i], PIPE_CONS_WARPS);
+    }
+    for (int i = 0; i < PIPE_TQ; i++) {
+      mbar_init(&bars->tq_full[i], 1);
+      mbar_init(&bars->tq_empty[i], PIPE_CONS_WARPS + PIPE_HALO_THREADS / 32);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+  const uint32_t link_bytes = (uint32_t)(NCU * TV * sizeof(T2<T>));
+  const uint32_t clv_bytes = (uint32_t)(HALF_CLV_ROWS * TV * sizeof(T2<T>));
+  const uint32_t sp_bytes = (uint32_t)(12 * TV * sizeof(T2<T>));
+
+  if (warp >= PIPE_CONS_WARPS) {
+    setmaxnreg_dec<56>();
+    if (warp == PIPE_CONS_WARPS) {
+      // ------------------------------ producer ------------------------------
+      if (lane == 0) {
+        const uint64_t pol_once = policy_evict_first();
+        RingPos rp = {0, 0u};
+        int k = 0, kt = 0;
+        int tile = blockIdx.x;
+        int tile_after = next_tile(g, a.sched, tile);
+        tq_push(bars, kt++, tile);
+        auto load_spinors = [&](const int t) {
+          mbar_arrive_expect_tx(&bars->full_sp, (SELF ? 2 : 1) * sp_bytes);
+          bulk_g2s(sp_in, a.in + field_offset(g, 12, q, t, 0, 0), sp_bytes, &bars->full_sp);
+          if (SELF) bulk_g2s(sp_self, a.self + field_offset(g, 12, p, t, 0, 0), sp_bytes, &bars->full_sp);
+        };
+        load_spinors(tile);
+        while (tile >= 0) {
+          tq_push(bars, kt++, tile_after);
+          const int tile_after2 = tile_after >= 0 ? next_tile(g, a.sched, tile_after) : -1;
+#pragma unroll 1
+          for (int st = 0; st < 4 + NSTC; st++) {   // L0 L1 L2 L3 C0 C1 C2 C3
+            mbar_wait_relaxed(&bars->empty[rp.slot], rp.ph ^ 1u);
+            T2<T>* dst = ring + rp.slot * 2 * NCU * TV;
+            if (st < 4) {
+              mbar_arrive_expect_tx(&bars->full[rp.slot], 2 * link_bytes);
+              for (int pp = 0; pp < 2; pp++)
+                bulk_g2s(dst + (pp * NCU) * TV, a.U + field_offset(g, 4 * NCU, pp, tile, st * NCU, 0), link_bytes, &bars->full[rp.slot]);
+            } else {   // blocks are read exactly once per application: evict-first
+              mbar_arrive_expect_tx(&bars->full[rp.slot], clv_bytes);
+              bulk_g2s_hint(dst, a.A + field_offset(g, 36, p, tile, (st - 4) * HALF_CLV_ROWS, 0), clv_bytes, &bars->full[rp.slot], pol_once);
+            }
+            rp.advance(nslot);
+          }
+          if (tile_after >= 0) {   // spinors of the next tile: the buffers are released after this tile's exchange
+            mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
+            load_spinors(tile_after);
+          }
+          k++;
+          tile = tile_after;
+          tile_after = tile_after2;
+        }
+      }
+    } else {
+      // ------------------------------ halo loaders ----------------------------
+      const int lt = tid - (PIPE_CONS_WARPS + 1) * 32;
+      RingPos hp = {0, 0u};
+      for (int kt = 0;; kt++) {
+        const int tile = tq_pop(bars, kt, lane);
+        if (tile < 0) break;
+        const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
+        for (int mu = 0; mu < 4; mu++) {
+          mbar_wait_relaxed(&bars->empty_h[hp.slot], hp.ph ^ 1u);
+          halo_load_half<T, NCU>(g, a, tab, mu, q, halo + hp.slot * HALF_NF, lt);
+          cp_async_arrive_noinc(&bars->full_h[hp.slot]);
+          hp.advance(HALF_NHB);
+        }
+      }
+    }
+  } else {
+    // ------------------------------ arithmetic ---------------------------------
+    setmaxnreg_inc<216>();
+    const int grp = warp >> 2;          // 0: forward hops, upper chirality; 1: backward hops, lower chirality
+    const int j = tid & (TV - 1);
+    int l[4];
+    l[1] = (j >> 1) & 3;
+    l[2] = (j >> 3) & 3;
+    l[3] = j >> 5;
+    l[0] = 2 * (j & 1) + ((p + l[1] + l[2] + l[3]) & 1);
+    const bool nonper = (g.bc != LQCD_BC_PERIODIC);
+    const T sg = a.dagger ? T(-1) : T(1);
+    RingPos rp = {0, 0u};
+    RingPos hp = {0, 0u};
+    double nrm = 0.0;
+    int k = 0;
+    for (int kt = 0;; kt++, k++) {
+      const int tile = tq_pop(bars, kt, lane);
+      if (tile < 0) break;
+      const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
+      const int x3 = __ldg(tab + 8) + l[3];
+      const bool live = !(nonper && frozen_slice(g, x3));
+      cx<T> acc[12];
+#pragma unroll
+      for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
+      mbar_wait(&bars->full_sp, (uint32_t)(k & 1));
+#define LQCD_HALF_HOP(MU)                                                                                              \
+      {                                                                                                                \
+        const int b = hp.slot;                                                                                         \
+        mbar_wait(&bars->full_h[b], hp.ph);                                                                            \
+        mbar_wait(&bars->full[rp.slot], rp.ph);                                                                        \
+        if (live) {                                                                                                    \
+          if (grp == 0) hop_one<T, RECON, MU, true>(g, a, sp_in, ring + rp.slot * 2 * NCU * TV, halo + b * HALF_NF, p, j, l, x3, nonper, sg, acc);  \
+          else hop_one<T, RECON, MU, false>(g, a, sp_in, ring + rp.slot * 2 * NCU * TV, halo + b * HALF_NF, p, j, l, x3, nonper, sg, acc);          \
+        }                                                                                                              \
+        release_fence();                                                                                               \
+        __syncwarp();                                                                                                  \
+        if (lane == 0) {                                                                                               \
+          mbar_arrive(&bars->empty[rp.slot]);                                                                          \
+          mbar_arrive(&bars->empty_h[b]);                                                                              \
+        }                                                                                                              \
+        rp.advance(nslot);                                                                                             \
+        hp.advance(HALF_NHB);                                                                                          \
+      }
+      LQCD_HALF_HOP(0)
+      LQCD_HALF_HOP(1)
+      LQCD_HALF_HOP(2)
+      LQCD_HALF_HOP(3)
+#undef LQCD_HALF_HOP
+      // swap halves through the input-spinor buffer (no hop reads it any more): rows 0-5 <- F's lower components,
+      // rows 6-11 <- B's upper components; then F adds B's upper half, B adds F's lower half.  From here on a thread
+      // holds ITS chirality in elements 0-5 of its arrays (register arrays want compile-time indices; the group only
+      // enters through addresses and selects).
+      cx<T> m[12], v[12];   // m: hop sums, later the accumulator of the block multiply; v: the vector the blocks act on
+      asm volatile("bar.sync 2, %0;" ::"n"(PIPE_CONS_WARPS * 32) : "memory");
+      {
+        T2<T>* x = sp_in + (grp == 0 ? 0 : 6) * TV + j;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          const cx<T> send(grp == 0 ? acc[6 + c].re : acc[c].re, grp == 0 ? acc[6 + c].im : acc[c].im);
+          m[c] = cx<T>(grp == 0 ? acc[c].re : acc[6 + c].re, grp == 0 ? acc[c].im : acc[6 + c].im);
+          st<T>(x + c * TV, send);
+        }
+      }
+      // these generic-proxy stores share their addresses with the next tile's bulk copy (async proxy): without the
+      // proxy fence the copy may overtake them (seen as a few garbage tiles per launch on a full grid)
+      fence_proxy_async();
+      asm volatile("bar.sync 2, %0;" ::"n"(PIPE_CONS_WARPS * 32) : "memory");
+      {
+        const T2<T>* x = sp_in + (grp == 0 ? 6 : 0) * TV + j;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          const T2<T> w = x[c * TV];
+          m[c] = cx<T>(m[c].re + w.x, m[c].im + w.y);
+        }
+      }
+      // this group's six components of the self spinor (before the buffers are released)
+      if (SELF) {
+        const T sc = (DIAG == DIAG_PRE) ? T(-1) / a.k : T(1);
+        const T2<T>* sv = sp_self + (grp == 0 ? 0 : 6) * TV + j;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          const T2<T> w = sv[c * TV];
+          v[c] = cx<T>(sc * w.x, sc * w.y);
+        }
+      }
+      release_fence();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->empty_sp);   // both spinor buffers may be overwritten
+      if (NSTC > 0) {
+        // DIAG_PRE: m = hops - (1/k) A self, result = -k m;  DIAG_POST: result = B (hops)
+        if (DIAG == DIAG_POST) {
+#pragma unroll
+          for (int c = 0; c < 6; c++) { v[c] = m[c]; m[c] = cx<T>(0, 0); }
+        }
+        // the packing of the two chiral blocks is the same: the stage of this group's chirality is processed as
+        // "chirality 0" on elements 0-5
+#define LQCD_HALF_CLV(S)                                                                                               \
+        {                                                                                                              \
+          mbar_wait(&bars->full[rp.slot], rp.ph);                                                                      \
+          if (live && grp == (S) / 2) CloverStage<T, ((S) & 1) * HALF_CLV_ROWS, HALF_CLV_ROWS>::run(ring + rp.slot * 2 * NCU * TV + j, TV, v, m);  \
+          release_fence();                                                                                             \
+          __syncwarp();                                                                                                \
+          if (lane == 0) mbar_arrive(&bars->empty[rp.slot]);                                                           \
+          rp.advance(nslot);                                                                                           \
+        }
+        LQCD_HALF_CLV(0)
+        LQCD_HALF_CLV(1)
+        LQCD_HALF_CLV(2)
+        LQCD_HALF_CLV(3)
+#undef LQCD_HALF_CLV
+      }
+      cx<T> res[6];
+#pragma unroll
+      for (int c = 0; c < 6; c++) {
+        if (!live) res[c] = cx<T>(0, 0);
+        else if (DIAG == DIAG_PRE) res[c] = cx<T>(-a.k * m[c].re, -a.k * m[c].im);
+        else if (DIAG == DIAG_POST) res[c] = m[c];
+        else res[c] = cx<T>(fma(-a.k, m[c].re, v[c].re), fma(-a.k, m[c].im, v[c].im));
+      }
+      // epilogue on this group's six components
+      const size_t ooff = field_offset(g, 12, p, tile, grp == 0 ? 0 : 6, j);
+      if (a.epi == EPI_AXPY_NORM) {
+        const T al = (T)(*a.alpha);
+        T2<T>* rq = a.r + ooff;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          T2<T> rv = rq[c * TV];
+          cx<T> w(fma(-al, res[c].re, rv.x), fma(-al, res[c].im, rv.y));
+          st<T>(rq + c * TV, w);
+          nrm += (double)w.re * (double)w.re + (double)w.im * (double)w.im;
+        }
+      } else {
+        T2<T>* op = a.out + ooff;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          st<T>(op + c * TV, res[c]);
+          if (a.epi == EPI_STORE_NORM) nrm += (double)res[c].re * (double)res[c].re + (double)res[c].im * (double)res[c].im;
+        }
+      }
+      if (a.epi != EPI_STORE) {   // one partial sum per tile, fixed order (see dw_pipe_kernel)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+        if (lane == 0) s_red[k & 1][warp] = nrm;
+        asm volatile("bar.sync 1, %0;" ::"n"(PIPE_CONS_WARPS * 32) : "memory");
+        if (tid == 0) {
+          double s = 0;
+          for (int w = 0; w < PIPE_CONS_WARPS; w++) s += s_red[k & 1][w];
+          a.partial[tile] = s;
+        }
+        nrm = 0.0;
+      }
+    }
+  }
+  if (a.sched != nullptr) {
+    if (tid == 0) {
       __threadfence();
       if (atomicAdd(a.sched + 1, 1u) == gridDim.x - 1) {
         a.sched[0] = 0u;
@@ -882,6 +1222,50 @@ static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
   return c;
 }
 
+// half-lattice pipeline (even-odd passes): DIAG_PRE / DIAG_POST on 4x4x4x4 tiles
+template <typename T>
+static PipeCfg pipe_half_config(const Geom& g, int recon, int diag, int parity) {
+  PipeCfg c = {false, 0, 0, 0};
+  if (dw_mode() != MODE_PIPE || parity < 0 || diag == DIAG_ONE) return c;
+  if (g.b[0] != 4 || g.b[1] != 4 || g.b[2] != 4 || g.b[3] != 4 || g.tile_tab == nullptr) return c;
+  if (env_int("LQCD_EO_PIPE", 1) == 0) return c;   // experiment switch: the one-thread-per-site kernel instead
+  const int ncu = recon == 12 ? 6 : 9;
+  const size_t sp = (size_t)(diag == DIAG_POST ? 12 : 24) * g.TV * sizeof(T2<T>);
+  const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
+  const size_t halo = (size_t)(24 + ncu) * HALF_HS * sizeof(T2<T>);
+  const size_t budget = (size_t)g.smem_optin - 256;
+  if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
+  int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
+  if (nslot > 4) nslot = 4;
+  const int e = env_int("LQCD_NSLOT", nslot);
+  if (e >= 2 && e <= nslot) nslot = e;
+  c.use = true;
+  c.nslot = nslot;
+  c.smem = sp + (size_t)nslot * slot + halo + sizeof(PipeBars);
+  c.grid = g.sm_count;
+  if (g_pipe_grid > 0 && g_pipe_grid < c.grid) c.grid = g_pipe_grid;
+  if (c.grid > g.ntiles) c.grid = g.ntiles;
+  return c;
+}
+
+static unsigned int* sched_slot(const Geom& g) {
+  static std::atomic<unsigned> launch_no(0);
+  // one pair of scheduler counters per launch in flight (a pool of SCHED_SLOTS pairs owned by the geometry, handed out
+  // round-robin): launches of the same geometry running concurrently on different streams do not share a counter
+  return (g.sched != nullptr && pipe_dynamic()) ? g.sched + 2 * (launch_no++ % SCHED_SLOTS) : nullptr;
+}
+
+template <typename T, int RECON, int DIAG>
+static cudaError_t launch_pipe_half(const Geom& g, const DwArgs<T>& a, const PipeCfg& c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(dw_pipe_half_kernel<T, RECON, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  DwArgs<T> b = a;
+  b.sched = sched_slot(g);
+  dw_pipe_half_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, b, c.nslot);
+  count_launch();
+  return cudaGetLastError();
+}
+
 template <typename T, int RECON, int DIAG>
 static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg& c, cudaStream_t s) {
   // the attribute is per function AND per device: set it on every launch (a host-side call of about a microsecond) rather
@@ -889,10 +1273,7 @@ static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg&
   cudaError_t e = cudaFuncSetAttribute(dw_pipe_kernel<T, RECON, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
   if (e != cudaSuccess) return e;
   DwArgs<T> b = a;
-  static std::atomic<unsigned> launch_no(0);
-  // one pair of scheduler counters per launch in flight (a pool of SCHED_SLOTS pairs owned by the geometry, handed out
-  // round-robin): launches of the same geometry running concurrently on different streams do not share a counter
-  b.sched = (g.sched != nullptr && pipe_dynamic()) ? g.sched + 2 * (launch_no++ % SCHED_SLOTS) : nullptr;
+  b.sched = sched_slot(g);
   dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, b, c.nslot);
   count_launch();
   return cudaGetLastError();
@@ -949,6 +1330,12 @@ template <typename T>
 void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int len) {
   const PipeCfg pc = pipe_config<T>(g, recon, diag, parity);
   const char* tn = sizeof(T) == 8 ? "double" : "float";
+  const PipeCfg hc = pipe_half_config<T>(g, recon, diag, parity);
+  if (hc.use) {
+    snprintf(buf, (size_t)len, "dw_pipe_half_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=3 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
+             tn, recon, diag, hc.grid, (int)PIPE_THREADS, hc.smem, hc.nslot, g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
+    return;
+  }
   if (pc.use) {
     snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=2 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
              tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
@@ -966,6 +1353,7 @@ template void dw_describe<float>(const Geom&, int, int, int, char*, int);
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity) {
   PipeCfg c = pipe_config<T>(g, recon, diag, parity);
+  if (!c.use) c = pipe_half_config<T>(g, recon, diag, parity);
   return c.use ? g.ntiles : direct_config<T>(g, recon, diag, parity).grid;   // pipeline: one partial sum per tile
 }
 template int dw_num_partials<double>(const Geom&, int, int, int);
@@ -1027,6 +1415,13 @@ cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cu
     if (c.use) {
       if (recon == 12) return diag == DIAG_ONE ? launch_pipe<T, 12, DIAG_ONE>(g, a, c, s) : launch_pipe<T, 12, DIAG_PRE>(g, a, c, s);
       return diag == DIAG_ONE ? launch_pipe<T, 18, DIAG_ONE>(g, a, c, s) : launch_pipe<T, 18, DIAG_PRE>(g, a, c, s);
+    }
+  }
+  if (a.parity >= 0 && a.nrhs <= 1) {
+    const PipeCfg c = pipe_half_config<T>(g, recon, diag, a.parity);
+    if (c.use) {
+      if (recon == 12) return diag == DIAG_PRE ? launch_pipe_half<T, 12, DIAG_PRE>(g, a, c, s) : launch_pipe_half<T, 12, DIAG_POST>(g, a, c, s);
+      return diag == DIAG_PRE ? launch_pipe_half<T, 18, DIAG_PRE>(g, a, c, s) : launch_pipe_half<T, 18, DIAG_POST>(g, a, c, s);
     }
   }
   if (a.nrhs > 1) {   // the one-thread-per-site kernels take one right-hand side per launch

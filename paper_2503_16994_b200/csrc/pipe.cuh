@@ -54,6 +54,17 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, uint32_t parity
   }
 }
 
+// orders this thread's earlier generic-proxy accesses to shared memory before later async-proxy ones (bulk copies issued
+// by whoever is released through a barrier afterwards)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Before a warp hands a shared-memory buffer back to the copy engine (arrive on its "empty" mbarrier) its own accesses
+// to that buffer must have been PERFORMED, not just issued: ptxas issues SYNCS.ARRIVE right behind the LDS of the
+// buffer (the arithmetic on the loaded values follows later) and the arrive can overtake them.  With bulk copies that
+// land a microsecond later this goes unnoticed; the half-lattice kernel, whose next spinor tile is requested the moment
+// the last warp arrives, showed it as a few overwritten tiles per launch.  membar.cta closes the window.
+__device__ __forceinline__ void release_fence() { __threadfence_block(); }
+
 // L2 eviction policy for bulk copies of data that is read exactly once (the clover blocks)
 __device__ __forceinline__ uint64_t policy_evict_first() {
   uint64_t p;

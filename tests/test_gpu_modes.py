@@ -92,7 +92,7 @@ def test_plan_and_option_errors():
     lat = Lattice((8, 8, 8, 8))
     assert "dw_pipe_kernel<double,18,1>" in B.dw_plan(lat.g)
     assert "ring_slots=3" in B.dw_plan(lat.g)                       # fp64: 3 x 36 KB stages + 2 x 33 KB halos + 48 KB tile
-    assert "dw_kernel_h<float,12,1,half>" in B.dw_plan(lat.g, B.F32, B.RECON_12, True, parity=1)   # half-lattice pass
+    assert "dw_pipe_half_kernel<float,12,1>" in B.dw_plan(lat.g, B.F32, B.RECON_12, True, parity=1)   # even-odd pass
     with pytest.raises(B.LqcdError):
         B.set_option("dw_mode", "bogus")
     with pytest.raises(B.LqcdError):
@@ -275,4 +275,74 @@ def test_no_write_outside_the_output(mode, prec):
     assert torch.all(dst_all[:G] == 0xA5) and torch.all(dst_all[G + nb:] == 0xA5)
     assert torch.equal(src_all, src_copy)
     assert torch.equal(lat.U[(prec, 18)], Ucopy) and torch.equal(lat.A[prec], Acopy)
+    lat.close()
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
+@pytest.mark.parametrize("L,bc,theta,phiT", CASES)
+@pytest.mark.parametrize("prec,recon", [(B.F64, B.RECON_18), (B.F64, B.RECON_12), (B.F32, B.RECON_18), (B.F32, B.RECON_12)])
+def test_dhat_parity_multi_tile(mode, L, bc, theta, phiT, prec, recon):
+    """Even-odd operator D^ = A_ee - kappa^2 H_eo A_oo^-1 H_oe (D8) and its dagger on lattices of several 4^4 tiles per
+    direction, every boundary condition: the half-lattice pipeline kernel (dw_pipe_half_kernel: forward / backward hops
+    on two warp groups, halves swapped through shared memory, one chirality of the block multiply per group) and the
+    one-thread-per-site kernel against oracle.dhat; also with one and three CTAs (every ring slot and phase)."""
+    kappa, csw = 0.1355, 1.8
+    U, psi = inputs(L, bc, 81)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc, phiT=phiT)
+    Ai = oracle.clover_inverse(L, A)
+    Uo, psio, Ao, Aio = (round_f32(U), round_f32(psi), round_f32(A), round_f32(Ai)) if prec == B.F32 else (U, psi, A, Ai)
+    x = np.arange(synth.vol(L))
+    par = np.zeros_like(x)
+    for mu in range(4):
+        par += x % L[mu]
+        x = x // L[mu]
+    even = (par % 2 == 0) & interior(L, bc)
+    lat = Lattice(L, bc, theta, synth.SF_PHI0, phiT)
+    lat.set_gauge(U, recons=(recon,), precs=(prec,))
+    lat.build_clover(kappa, csw, recon=recon, precs=(prec,), inverse=True)
+    plan = B.dw_plan(lat.g, prec, recon, True, parity=0)
+    assert ("dw_pipe_half_kernel" in plan) == (mode == "pipe"), plan
+    src = lat.spinor(psi, prec)
+    tmp = lat.alloc(B.FIELD_SPINOR, prec)
+    try:
+        for grid in ((0, 1, 3) if mode == "pipe" else (0,)):
+            B.set_option("pipe_grid", str(grid))
+            for dagger in (False, True):
+                ref = oracle.dhat(L, Uo, psio, kappa, Ao, Aio, bc=bc, theta=theta, dagger=dagger)
+                dst = lat.alloc(B.FIELD_SPINOR, prec)
+                dst.zero_()
+                B.dw_eo_apply(lat.g, kappa, lat.U[(prec, recon)], lat.A[prec], lat.Ainv[prec], src, dst, tmp, dagger, prec, recon)
+                got = lat.spinor_to_host(dst, prec)
+                assert site_rel_err(got, ref, even) <= TOL[prec] * 2, (grid, dagger)
+                frozen_even = (par % 2 == 0) & ~interior(L, bc)
+                assert np.all(got[frozen_even] == 0)
+    finally:
+        B.set_option("pipe_grid", "0")
+    lat.close()
+
+
+@pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
+@pytest.mark.parametrize("mixed", [False, True])
+def test_cg_eo_multi_tile(mode, mixed):
+    """The even-odd solver (fused epilogues of the half-lattice kernels; fp32 inner solver when mixed) on a lattice of
+    32 tiles with open boundaries against the oracle's CG."""
+    L, bc, kappa, csw = (8, 8, 8, 16), B.BC_OPEN, 0.13, 1.7
+    U, _ = inputs(L, bc, 85)
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
+    precs = (B.F64, B.F32) if mixed else (B.F64,)
+    lat = Lattice(L, bc)
+    lat.set_gauge(U, precs=precs)
+    lat.build_clover(kappa, csw, precs=precs, inverse=True)
+    b = synth.point_source(L, (1, 2, 3, 8), 2, 0)
+    xo, it_o, _, rt_o = oracle.cg(L, U, b, kappa, A, bc=bc, tol=1e-10)
+    x, ws = lat.alloc(B.FIELD_SPINOR), lat.alloc(B.FIELD_WORKSPACE)
+    kw = dict(U32=lat.U[(B.F32, 18)], clover32=lat.A[B.F32], clover_inv32=lat.Ainv[B.F32]) if mixed else {}
+    info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], lat.spinor(b), x, ws, tol=1e-10, maxiter=5000,
+                      clover_inv64=lat.Ainv[B.F64], eo=True, mixed=mixed, **kw)
+    assert info["status"] == B.OK
+    got = lat.spinor_to_host(x)
+    rt = np.linalg.norm(b - oracle.dw(L, U, got, kappa, A, bc=bc))
+    assert rt <= 50e-10 and abs(info["rel_resid_true"] - rt) <= 0.5 * rt + 1e-13
+    assert np.linalg.norm(got - xo) / np.linalg.norm(xo) <= 200 * (rt + rt_o)
+    assert np.all(got[~interior(L, bc)] == 0)
     lat.close()
