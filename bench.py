@@ -565,13 +565,17 @@ def run_config3(torch, B, synth, peak):
     y = (0, 0, 0, L[3] // 2)   # R12: slice 0 is frozen under open BC
     out = {}
     for name, kw in (("plain_f64", {}),
-                     ("eo_mixed", dict(eo=True, mixed=True, clover_inv64=S.Ainv[B.F64], U32=U32, clover32=S.A[B.F32],
-                                       clover_inv32=S.Ainv[B.F32]))):
+                     # inner_tol 1e-2: on this ill-conditioned lattice an fp32 inner solve of ~1500 iterations ends with a
+                     # recursive residual far below its true one, and asking it for 1e-4 sometimes buys a second such
+                     # solve that makes no progress (DESIGN.md section 7 "Mixed precision")
+                     ("eo_mixed", dict(eo=True, mixed=True, inner_tol=1e-2, clover_inv64=S.Ainv[B.F64], U32=U32,
+                                       clover32=S.A[B.F32], clover_inv32=S.Ainv[B.F32]))):
         t0 = time.perf_counter()
         infos = B.propagator(g, kappa, S.U[(B.F64, 18)], S.A[B.F64], y, cols, ws, tol=1e-10, maxiter=10000, **kw)
         dt = time.perf_counter() - t0
         out["a8_propagator_24x24x24x48_open_" + name] = {
             "seconds_12_columns": round(dt, 3), "iterations": [i["iters"] for i in infos],
+            "outer": [i["outer"] for i in infos],
             "max_rel_resid_normal": max(i["rel_resid_normal"] for i in infos),
             "max_rel_resid_true": max(i["rel_resid_true"] for i in infos)}
     S.close()

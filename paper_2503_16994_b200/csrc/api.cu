@@ -672,6 +672,9 @@ lqcd_status solve_normal(const SolveCtx& c, const void* bp, void* x, int* iters,
     CKS(cg_normal<float>(M32, c.v32[0], c.v32[5], w, itol, c.parm->maxiter - total, check, &hs, c.s), "cg_normal32");
     total += hs.iters;
     *outer += 1;
+    if (getenv("LQCD_CG_VERBOSE"))
+      fprintf(stderr, "lqcd_cg_solve mixed: outer %d: |r|/|b'| = %.3e before, inner tol %.1e, inner iterations %d (inner recursive |r|^2 ratio %.3e)\n",
+              *outer, sqrt(rho / rho0), itol, hs.iters, hs.rho0 > 0 ? hs.rho / hs.rho0 : 0.0);
     if (hs.breakdown) { *iters = total; set_error("lqcd_cg_solve: breakdown in the fp32 inner solve"); return LQCD_EBREAKDOWN; }
     CKS(add_f32_to_f64(c.v32[5], x, n, c.s), "x += e");
     CKS(M.apply(x, t64, false, EPI_STORE, nullptr, nullptr, nullptr, nullptr, c.s), "M x");
