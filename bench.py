@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-rows", action="store_true", help="skip the per-row extras (rank 0, N=1)")
+    ap.add_argument("--rows", default="main,config2,config3,config4,config5b",
+                    help="which groups of rows to measure: main (the other rows on the timed lattice), config2, config3, "
+                         "config4, config5b")
     ap.add_argument("--decompose", action="store_true",
                     help="NEXT-3 (opt-in, not the driver's mode): ONE lattice cut into --gpus time slabs, half-spinor "
                          "faces exchanged between ring neighbours (NCCL); strong scaling")
@@ -319,13 +322,13 @@ def run_ours(args):
 # running library describes its launch differently, i.e. when the kernel or its tiling changed since the capture.
 NCU_TRAFFIC = {
     ("48x48x48x96", "f64", 18): {
-        "bytes": 15717323000 + 2025048000,
+        "bytes": 15727609000 + 2025297999,
         "capture": "profiles/r02_dw_pipe_kernel_f64_full.txt",
-        "plan": "dw_pipe_kernel<double,18,1> grid=148 threads=384 smem=227648 ring_slots=3 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
+        "plan": "dw_pipe_kernel<double,18,1> grid=148 threads=384 smem=227680 ring_slots=3 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
     ("48x48x48x96", "f32", 18): {
         "bytes": 8046293000 + 1009103000,
         "capture": "profiles/r02_dw_pipe_kernel_f32_full.txt",
-        "plan": "dw_pipe_kernel<float,18,1> grid=148 threads=384 smem=132416 ring_slots=4 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
+        "plan": "dw_pipe_kernel<float,18,1> grid=148 threads=384 smem=132448 ring_slots=4 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
 }
 
 
@@ -384,6 +387,12 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
     """The other hot-path rows measured once each, same process, rank 0, N = 1."""
     rows = {}
     V, L, g, kappa = S.V, S.L, S.g, args.kappa
+    groups = set(args.rows.split(","))
+    if "main" not in groups:
+        for name, fn in (("config2", run_config2), ("config3", run_config3), ("config4", run_config4), ("config5b", run_config5b)):
+            if name in groups:
+                rows.update(fn(torch, B, synth, peak))
+        return rows
 
     def gbs(reals, rbytes, ms, sites=V):
         return round(reals * rbytes * sites / (ms * 1e-3) / 1e9, 1)
@@ -488,10 +497,9 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
         B.geom_destroy(gs)
     del ws
     torch.cuda.empty_cache()
-    rows.update(run_config2(torch, B, synth, peak))
-    rows.update(run_config3(torch, B, synth, peak))
-    rows.update(run_config4(torch, B, synth, peak))
-    rows.update(run_config5b(torch, B, synth, peak))
+    for name, fn in (("config2", run_config2), ("config3", run_config3), ("config4", run_config4), ("config5b", run_config5b)):
+        if name in groups:
+            rows.update(fn(torch, B, synth, peak))
     return rows
 
 
