@@ -18,12 +18,17 @@ _LIB = os.path.join(_HERE, "liblqcd_oracle.so")
 BC_PERIODIC, BC_OPEN, BC_SF_ORBI, BC_SF_AFWB = 0, 1, 2, 3
 
 
+_SRC_SUN = os.path.join(_HERE, "lqcd_oracle_sun.cpp")
+_LIB_SUN = os.path.join(_HERE, "liblqcd_oracle_sun.so")
+
+
 def build(force=False):
-    """Compile the oracle with g++ -O2 -fopenmp (no fast-math: fp64 results must be plain IEEE)."""
-    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
-        return _LIB
-    cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC]
-    subprocess.check_call(cmd)
+    """Compile the oracles with g++ -O2 -fopenmp (no fast-math: fp64 results must be plain IEEE): the SU(3) oracle
+    and, separately, the N-colour oracle of the SU(2) fundamental representation."""
+    for src, lib_ in ((_SRC, _LIB), (_SRC_SUN, _LIB_SUN)):
+        if not force and os.path.exists(lib_) and os.path.getmtime(lib_) >= os.path.getmtime(src):
+            continue
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", lib_, src])
     return _LIB
 
 
@@ -219,3 +224,79 @@ def correlator_ps(L, cols):
     C = np.zeros(int(L[3]), dtype=np.float64)
     lib().oracle_correlator_ps(_L(L), _p(cols), ctypes.c_int(cols.shape[0]), _p(C))
     return C
+
+
+# ---- SU(2) fundamental representation (PAPER.md:66-70): the N-colour oracle of lqcd_oracle_sun.cpp -------------------
+# gauge [V,4,N,N], spinor [V,4,N], blocks [V,2,2N,2N]; nc = 2 is the representation under test, nc = 3 exists to pin
+# the generic loops against the SU(3) oracle above.
+_lib_sun = None
+
+
+def lib_sun():
+    global _lib_sun
+    if _lib_sun is None:
+        build()
+        _lib_sun = ctypes.CDLL(_LIB_SUN)
+    return _lib_sun
+
+
+def su2_from_cayley_dickson(z):
+    """[..., 2] Cayley-Dickson pairs (z1, z2) -> [..., 2, 2] matrices [[z1, z2], [-conj z2, conj z1]]."""
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    out = np.zeros(z.shape[:-1] + (2, 2), dtype=np.complex128)
+    lib_sun().oracle_su2_from_cayley_dickson(ctypes.c_long(z.size // 2), _p(z), _p(out))
+    return out
+
+
+def sun_dw(nc, L, U, psi, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, dagger=False):
+    U = _c(U, (vol(L), 4, nc, nc))
+    psi = _c(psi, (vol(L), 4, nc))
+    out = np.zeros_like(psi)
+    ap = None
+    if Ablk is not None:
+        Ablk = _c(Ablk, (vol(L), 2, 2 * nc, 2 * nc))
+        ap = _p(Ablk)
+    rc = lib_sun().oracle_sun_dw(ctypes.c_int(nc), _L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap,
+                                 _p(psi), _p(out), ctypes.c_int(1 if dagger else 0))
+    assert rc == 0
+    return out
+
+
+def sun_hop(nc, L, U, psi, bc=BC_PERIODIC, theta=None):
+    U = _c(U, (vol(L), 4, nc, nc))
+    psi = _c(psi, (vol(L), 4, nc))
+    out = np.zeros_like(psi)
+    assert lib_sun().oracle_sun_hop(ctypes.c_int(nc), _L(L), ctypes.c_int(bc), _d(theta, 4), _p(U), _p(psi), _p(out)) == 0
+    return out
+
+
+def sun_fhat_site(nc, L, U, x, mu, nu):
+    U = _c(U, (vol(L), 4, nc, nc))
+    out = np.zeros((nc, nc), dtype=np.complex128)
+    assert lib_sun().oracle_sun_fhat_site(ctypes.c_int(nc), _L(L), _p(U), _L(x), ctypes.c_int(mu), ctypes.c_int(nu), _p(out)) == 0
+    return out
+
+
+def sun_clover_blocks(nc, L, U, kappa, csw, bc=BC_PERIODIC):
+    U = _c(U, (vol(L), 4, nc, nc))
+    out = np.zeros((vol(L), 2, 2 * nc, 2 * nc), dtype=np.complex128)
+    assert lib_sun().oracle_sun_clover_blocks(ctypes.c_int(nc), _L(L), ctypes.c_int(bc), ctypes.c_double(kappa),
+                                              ctypes.c_double(csw), _p(U), _p(out)) == 0
+    return out
+
+
+def sun_cg(nc, L, U, b, kappa, Ablk=None, bc=BC_PERIODIC, theta=None, tol=1e-10, maxiter=10000):
+    """Returns (x, iters, rel_resid_normal, rel_resid_true); iters < 0 means maxiter was hit."""
+    U = _c(U, (vol(L), 4, nc, nc))
+    b = _c(b, (vol(L), 4, nc))
+    x = np.zeros_like(b)
+    ap = None
+    if Ablk is not None:
+        Ablk = _c(Ablk, (vol(L), 2, 2 * nc, 2 * nc))
+        ap = _p(Ablk)
+    rn, rt = ctypes.c_double(0), ctypes.c_double(0)
+    f = lib_sun().oracle_sun_cg
+    f.restype = ctypes.c_int
+    it = f(ctypes.c_int(nc), _L(L), ctypes.c_int(bc), _d(theta, 4), ctypes.c_double(kappa), _p(U), ap, _p(b), _p(x),
+           ctypes.c_double(tol), ctypes.c_int(maxiter), ctypes.byref(rn), ctypes.byref(rt))
+    return x, int(it), rn.value, rt.value
