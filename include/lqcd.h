@@ -256,6 +256,34 @@ const char* lqcd_last_error(void);
 /* number of kernels launched by this library since load (for bench.py's gpu_launches) */
 long long lqcd_launch_count(void);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * The SU(2) fundamental representation (section 2.2: gauge fields in SU2{T},
+ * stored in the Cayley-Dickson form g = (z1, z2), |z1|^2 + |z2|^2 = 1; fermion fields Spinor{4, SU2fund}).
+ * Same geometry handle, same definitions D1-D8 with two colours, same tile-blocked layout; per site 8 complex numbers
+ * of links (4 directions x (z1, z2); U = [[z1, z2], [-conj z2, conj z1]]), 8 of spinor (index 2*spin + colour) and 16
+ * of clover term (two packed Hermitian 4x4 blocks, row index 2*s + a).  Canonical (interchange) layouts, DEVICE
+ * memory, complex fp64: gauge [V][4][2][2] (full matrices; import keeps the first row), spinor [V][4][2], blocks
+ * [V][2][4][4].  Periodic and open time boundaries (LQCD_EUNSUPPORTED-like LQCD_EINVAL otherwise); mu = 0, ct = 1;
+ * no even-odd or mixed-precision solver.  One-thread-per-site kernels (the shared-memory pipeline is SU(3) only).
+ * lqcd_su2_field_bytes: GAUGE | SPINOR | CLOVER | WORKSPACE (of lqcd_su2_cg_solve).  All calls are asynchronous on
+ * `stream` except lqcd_su2_cg_solve (PAPER.md:125 CG!, :171-172: maxiter, tol, iteration count), which follows
+ * lqcd_cg_solve: x0 = 0, stop when |r| <= tol |D^+ b| (recursive residual), true residuals in `info`, LQCD_ENOTCONV
+ * with the last iterate in x when maxiter is hit, components of b on frozen slices ignored. */
+size_t lqcd_su2_field_bytes(const lqcd_geom* g, lqcd_field_kind kind, lqcd_prec prec);
+lqcd_status lqcd_su2_gauge_import(const lqcd_geom* g, const void* canon, void* U, lqcd_prec prec, void* stream);
+lqcd_status lqcd_su2_gauge_export(const lqcd_geom* g, const void* U, void* canon, lqcd_prec prec, void* stream);
+lqcd_status lqcd_su2_spinor_import(const lqcd_geom* g, const void* canon, void* psi, lqcd_prec prec, void* stream);
+lqcd_status lqcd_su2_spinor_export(const lqcd_geom* g, const void* psi, void* canon, lqcd_prec prec, void* stream);
+/* Csw! from the fp64 links; the blocks are rounded once to out_prec (R14) */
+lqcd_status lqcd_su2_clover_build(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, void* clover, lqcd_prec out_prec,
+                                  void* stream);
+lqcd_status lqcd_su2_clover_export(const lqcd_geom* g, const void* clover, void* canon, lqcd_prec prec, void* stream);
+/* Dw!: out = D in (dagger = 0) or D^+ in; clover = NULL means csw = 0; out must not alias an input */
+lqcd_status lqcd_su2_dw_apply(const lqcd_geom* g, const lqcd_dirac* d, const void* U, const void* clover, const void* in,
+                              void* out, int dagger, lqcd_prec prec, void* stream);
+lqcd_status lqcd_su2_cg_solve(const lqcd_geom* g, const lqcd_dirac* d, const void* U64, const void* clover64, const void* b,
+                              void* x, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

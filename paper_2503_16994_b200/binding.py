@@ -26,6 +26,8 @@ EXPORTS = [
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_host_cache_release", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
     "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
     "lqcd_clover_build_slab", "lqcd_cg_solve_slab",
+    "lqcd_su2_field_bytes", "lqcd_su2_gauge_import", "lqcd_su2_gauge_export", "lqcd_su2_spinor_import",
+    "lqcd_su2_spinor_export", "lqcd_su2_clover_build", "lqcd_su2_clover_export", "lqcd_su2_dw_apply", "lqcd_su2_cg_solve",
 ]
 
 
@@ -342,3 +344,54 @@ def dw_plan(g, prec=F64, recon=RECON_18, has_clover=True, parity=-1):
 
 def set_option(key, value):
     _check(lib().lqcd_set_option(key.encode(), value.encode()))
+
+
+# ---- SU(2) fundamental representation (NEXT-4; include/lqcd.h "The SU(2) fundamental representation") ---------------
+def su2_alloc_field(g, kind, prec=F64):
+    import torch
+    lib().lqcd_su2_field_bytes.restype = ctypes.c_size_t
+    n = lib().lqcd_su2_field_bytes(g, kind, prec)
+    return torch.empty(n, dtype=torch.uint8, device="cuda")
+
+
+def su2_gauge_import(g, canon, U, prec=F64, stream=None):
+    _check(lib().lqcd_su2_gauge_import(g, _ptr(canon), _ptr(U), prec, _stream(stream)))
+
+
+def su2_gauge_export(g, U, canon, prec=F64, stream=None):
+    _check(lib().lqcd_su2_gauge_export(g, _ptr(U), _ptr(canon), prec, _stream(stream)))
+
+
+def su2_spinor_import(g, canon, psi, prec=F64, stream=None):
+    _check(lib().lqcd_su2_spinor_import(g, _ptr(canon), _ptr(psi), prec, _stream(stream)))
+
+
+def su2_spinor_export(g, psi, canon, prec=F64, stream=None):
+    _check(lib().lqcd_su2_spinor_export(g, _ptr(psi), _ptr(canon), prec, _stream(stream)))
+
+
+def su2_clover_build(g, kappa, csw, U64, clover, prec=F64, stream=None):
+    d = _dirac(kappa, csw)
+    _check(lib().lqcd_su2_clover_build(g, ctypes.byref(d), _ptr(U64), _ptr(clover), prec, _stream(stream)))
+
+
+def su2_clover_export(g, clover, canon, prec=F64, stream=None):
+    _check(lib().lqcd_su2_clover_export(g, _ptr(clover), _ptr(canon), prec, _stream(stream)))
+
+
+def su2_dw_apply(g, kappa, U, clover, src, dst, dagger=False, prec=F64, stream=None):
+    d = _dirac(kappa)
+    _check(lib().lqcd_su2_dw_apply(g, ctypes.byref(d), _ptr(U), _ptr(clover), _ptr(src), _ptr(dst), 1 if dagger else 0, prec,
+                                   _stream(stream)))
+
+
+def su2_cg_solve(g, kappa, U64, clover64, b, x, workspace, tol=1e-10, maxiter=10000, check_every=16, stream=None,
+                 raise_on_notconv=True):
+    d = _dirac(kappa)
+    f, p = _cg_args(U64, clover64, None, None, None, None, tol, maxiter, False, False, 1e-4, check_every)
+    info = CgInfo()
+    st = lib().lqcd_su2_cg_solve(g, ctypes.byref(d), _ptr(U64), _ptr(clover64), _ptr(b), _ptr(x), _ptr(workspace), ctypes.byref(p),
+                                 ctypes.byref(info), _stream(stream))
+    if st != OK and not (st == ENOTCONV and not raise_on_notconv):
+        _check(st)
+    return _info_dict(info, st)

@@ -1144,3 +1144,156 @@ extern "C" lqcd_status lqcd_dw_apply_host(const lqcd_geom_desc* desc, const lqcd
   return LQCD_OK;
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// SU(2) fundamental representation
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+bool su2_bc_ok(const lqcd_geom* h) { return h->g.bc == LQCD_BC_PERIODIC || h->g.bc == LQCD_BC_OPEN; }
+size_t su2_spinor_complex(const Geom& g) { return (size_t)2 * g.Vh * 8; }
+}  // namespace
+#define SU2_COMMON(h, d, name)                                                                                      \
+  do {                                                                                                             \
+    REQUIRE(su2_bc_ok(h), name ": SU(2) fields support periodic and open time boundaries only");                  \
+    if (d) {                                                                                                       \
+      REQUIRE(good_kappa((const lqcd_dirac*)(d)), name ": kappa must be positive and finite");                    \
+      REQUIRE(((const lqcd_dirac*)(d))->mu == 0.0 && ((const lqcd_dirac*)(d))->ct == 1.0, name ": mu = 0 and ct = 1 only in the SU(2) representation"); \
+    }                                                                                                              \
+  } while (0)
+
+extern "C" {
+
+size_t lqcd_su2_field_bytes(const lqcd_geom* h, lqcd_field_kind kind, lqcd_prec prec) {
+  if (!h) return 0;
+  const Geom& g = h->g;
+  const size_t sites = (size_t)2 * g.Vh, eb = elem_bytes(prec);
+  switch (kind) {
+    case LQCD_FIELD_GAUGE: return sites * 8 * eb;
+    case LQCD_FIELD_SPINOR: return sites * 8 * eb;
+    case LQCD_FIELD_CLOVER: return sites * 16 * eb;
+    case LQCD_FIELD_WORKSPACE: return 6 * align256(sites * 8 * sizeof(double2)) + 2 * align256(partial_len(g) * sizeof(double)) + 4096;
+    default: return 0;
+  }
+}
+lqcd_status lqcd_su2_gauge_import(const lqcd_geom* h, const void* canon, void* U, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && U && canon != U, "lqcd_su2_gauge_import: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_gauge_import: bad precision");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_gauge_import<double>(h->g, canon, U, as_stream(stream)), su2_gauge_import<float>(h->g, canon, U, as_stream(stream))), "su2_gauge_import");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_gauge_export(const lqcd_geom* h, const void* U, void* canon, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && U && canon != U, "lqcd_su2_gauge_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_gauge_export: bad precision");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_gauge_export<double>(h->g, U, canon, as_stream(stream)), su2_gauge_export<float>(h->g, U, canon, as_stream(stream))), "su2_gauge_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_spinor_import(const lqcd_geom* h, const void* canon, void* psi, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && psi && canon != psi, "lqcd_su2_spinor_import: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_spinor_import: bad precision");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_spinor_import<double>(h->g, canon, psi, as_stream(stream)), su2_spinor_import<float>(h->g, canon, psi, as_stream(stream))), "su2_spinor_import");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_spinor_export(const lqcd_geom* h, const void* psi, void* canon, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && psi && canon != psi, "lqcd_su2_spinor_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_spinor_export: bad precision");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_spinor_export<double>(h->g, psi, canon, as_stream(stream)), su2_spinor_export<float>(h->g, psi, canon, as_stream(stream))), "su2_spinor_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_clover_build(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, void* clover, lqcd_prec out_prec, void* stream) {
+  REQUIRE(h && d && U64 && clover && clover != U64, "lqcd_su2_clover_build: NULL or aliased argument");
+  REQUIRE(valid_prec(out_prec), "lqcd_su2_clover_build: bad precision");
+  SU2_COMMON(h, d, "lqcd_su2_clover_build");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(out_prec, su2_clover_build<double>(h->g, d->kappa, d->csw, U64, clover, as_stream(stream)),
+                         su2_clover_build<float>(h->g, d->kappa, d->csw, U64, clover, as_stream(stream))), "su2_clover_build");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_clover_export(const lqcd_geom* h, const void* clover, void* canon, lqcd_prec prec, void* stream) {
+  REQUIRE(h && canon && clover && canon != clover, "lqcd_su2_clover_export: NULL or aliased argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_clover_export: bad precision");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_clover_export<double>(h->g, clover, canon, as_stream(stream)), su2_clover_export<float>(h->g, clover, canon, as_stream(stream))), "su2_clover_export");
+  return LQCD_OK;
+}
+lqcd_status lqcd_su2_dw_apply(const lqcd_geom* h, const lqcd_dirac* d, const void* U, const void* clover, const void* in, void* out,
+                              int dagger, lqcd_prec prec, void* stream) {
+  REQUIRE(h && d && U && in && out, "lqcd_su2_dw_apply: NULL argument");
+  REQUIRE(valid_prec(prec), "lqcd_su2_dw_apply: bad precision");
+  REQUIRE(out != in && out != U && out != clover, "lqcd_su2_dw_apply: output aliases an input");
+  SU2_COMMON(h, d, "lqcd_su2_dw_apply");
+  DeviceGuard dg(h);
+  CUDA_TRY(DISPATCH_PREC(prec, su2_dw<double>(h, d->kappa, U, clover, in, out, dagger != 0, as_stream(stream)),
+                         su2_dw<float>(h, d->kappa, U, clover, in, out, dagger != 0, as_stream(stream))), "su2_dw kernel");
+  return LQCD_OK;
+}
+
+// CG on D^+ D x = D^+ b in fp64 (the algorithm of lqcd_cg_solve, unfused BLAS-1, scalars on the device)
+lqcd_status lqcd_su2_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const void* U64, const void* clover64, const void* b, void* x,
+                              void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* info, void* stream) {
+  REQUIRE(h && d && U64 && b && x && workspace && parm && info, "lqcd_su2_cg_solve: NULL argument");
+  REQUIRE(x != b, "lqcd_su2_cg_solve: x aliases b");
+  REQUIRE(parm->tol > 0 && parm->maxiter >= 0 && !parm->eo && !parm->mixed, "lqcd_su2_cg_solve: bad tol / maxiter, or eo / mixed (not available for SU(2))");
+  SU2_COMMON(h, d, "lqcd_su2_cg_solve");
+  DeviceGuard dg(h);
+  memset(info, 0, sizeof(*info));
+  auto t0 = std::chrono::steady_clock::now();
+  const Geom& g = h->g;
+  cudaStream_t s = as_stream(stream);
+  const size_t n = su2_spinor_complex(g), bytes = n * sizeof(double2);
+  Workspace ws{(char*)workspace, 0};
+  void *r = ws.take(bytes), *p = ws.take(bytes), *t = ws.take(bytes), *q = ws.take(bytes), *bp = ws.take(bytes), *bm = ws.take(bytes);
+  double* partial = (double*)ws.take(partial_len(g) * sizeof(double));
+  double* scratch = (double*)ws.take(64);
+  CgState* state = (CgState*)ws.take(sizeof(CgState));
+  const int nb = reduce_blocks(n);
+  auto D = [&](const void* in, void* out, bool dag) { return su2_dw<double>(h, d->kappa, U64, clover64, in, out, dag, s); };
+  CKS(cudaMemcpyAsync(bm, b, bytes, cudaMemcpyDeviceToDevice, s), "copy b");
+  if (g.bc != LQCD_BC_PERIODIC) CKS(su2_mask_frozen<double>(g, bm, s), "mask");   // D7: the solve lives on the interior
+  CKS(D(bm, bp, true), "D^+ b");
+  CKS(cudaMemsetAsync(x, 0, bytes, s), "memset");
+  CKS(cudaMemcpyAsync(r, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+  CKS(cudaMemcpyAsync(p, bp, bytes, cudaMemcpyDeviceToDevice, s), "copy");
+  CKS(norm2_partial<double>(r, n, partial, s), "norm2");
+  CKS(cg_init_state(state, partial, nb, parm->tol, s), "cg_init_state");
+  const int check = parm->check_every > 0 ? parm->check_every : 16;
+  CgState hs;
+  int launched = 0;
+  for (;;) {
+    CKS(cudaMemcpyAsync(&hs, state, sizeof(CgState), cudaMemcpyDeviceToHost, s), "copy state");
+    CKS(cudaStreamSynchronize(s), "sync");
+    if (hs.done || launched >= parm->maxiter) break;
+    int batch = check;
+    if (launched + batch > parm->maxiter) batch = parm->maxiter - launched;
+    for (int it = 0; it < batch; it++) {
+      CKS(D(p, t, false), "D p");
+      CKS(norm2_partial<double>(t, n, partial, s), "norm2");
+      CKS(cg_reduce_alpha(state, partial, nb, s), "alpha");
+      CKS(D(t, q, true), "D^+ t");
+      CKS(cg_raxpy_norm<double>(state, q, r, n, partial, s), "r -= alpha q");
+      CKS(cg_reduce_beta(state, partial, nb, s), "beta");
+      CKS(cg_update_xp<double>(state, x, p, r, n, s), "update");
+    }
+    launched += batch;
+  }
+  info->iters = hs.iters;
+  // true residuals with fresh operator applications (R11)
+  double nbv = 0, nr = 0, nq = 0;
+  CKS(D(x, t, false), "D x");
+  CKS(xmy<double>(bm, t, t, n, s), "b - Dx");
+  CKS(device_norm2<double>(bm, n, partial, scratch, &nbv, s), "norm2");
+  CKS(device_norm2<double>(t, n, partial, scratch, &nr, s), "norm2");
+  CKS(D(t, q, true), "D^+ (b - Dx)");
+  CKS(device_norm2<double>(q, n, partial, scratch, &nq, s), "norm2");
+  info->rel_resid_true = nbv > 0 ? sqrt(nr / nbv) : 0.0;
+  info->rel_resid_normal = hs.rho0 > 0 ? sqrt(nq / hs.rho0) : 0.0;
+  info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  if (hs.breakdown) { set_error("lqcd_su2_cg_solve: breakdown (NaN or <p,D^+D p> <= 0) at iteration %d", hs.iters); return LQCD_EBREAKDOWN; }
+  if (!hs.done) { set_error("lqcd_su2_cg_solve: not converged after %d iterations", hs.iters); return LQCD_ENOTCONV; }
+  return LQCD_OK;
+}
+
+}  // extern "C"

@@ -29,6 +29,18 @@ cudaError_t clover_build(const Geom& g, const CloverParm& cp, const void* U64, i
 }  // namespace lqcd
 struct lqcd_geom;
 namespace lqcd {
+// su2.cu -- the SU(2) fundamental representation (NEXT-4): Cayley-Dickson links (8 complex per site), 4 x 2 spinors (8),
+// two packed Hermitian 4x4 blocks (16)
+template <typename T> cudaError_t su2_gauge_import(const Geom& g, const void* canon, void* U, cudaStream_t s);
+template <typename T> cudaError_t su2_gauge_export(const Geom& g, const void* U, void* canon, cudaStream_t s);
+template <typename T> cudaError_t su2_spinor_import(const Geom& g, const void* canon, void* psi, cudaStream_t s);
+template <typename T> cudaError_t su2_spinor_export(const Geom& g, const void* psi, void* canon, cudaStream_t s);
+template <typename T> cudaError_t su2_clover_build(const Geom& g, double kappa, double csw, const void* U64, void* A, cudaStream_t s);
+template <typename T> cudaError_t su2_clover_export(const Geom& g, const void* A, void* canon, cudaStream_t s);
+template <typename T> cudaError_t su2_dw(const lqcd_geom* h, double kappa, const void* U, const void* A, const void* in, void* out, bool dagger, cudaStream_t s);
+template <typename T> cudaError_t su2_mask_frozen(const Geom& g, void* psi, cudaStream_t s);
+}  // namespace lqcd
+namespace lqcd {
 template <typename T> cudaError_t slab_pack(const lqcd_geom* h, bool dagger, const void* U, int recon, const void* in,
                                             void* send_lo, void* send_hi, cudaStream_t s);
 template <typename T> cudaError_t slab_faces(const lqcd_geom* h, double kappa, bool dagger, const void* U, int recon,
