@@ -497,10 +497,45 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
         B.geom_destroy(gs)
     del ws
     torch.cuda.empty_cache()
+    if "main" in groups:
+        rows.update(run_su2(torch, B, synth, peak, L))
     for name, fn in (("config2", run_config2), ("config3", run_config3), ("config4", run_config4), ("config5b", run_config5b)):
         if name in groups:
             rows.update(fn(torch, B, synth, peak))
     return rows
+
+
+def run_su2(torch, B, synth, peak, L):
+    """NEXT-4: the SU(2) fundamental representation on the bench lattice -- Dw in fp64 and
+    fp32 (one-thread-per-site kernel).  Compulsory bytes per site: 16 link reals (Cayley-Dickson pairs) + 16 psi in +
+    16 out + 32 clover = 80 reals; flops: hopping 624 + block multiply 208 + combine 32 = 864 per site."""
+    import numpy as np
+    kappa, csw = 0.137, 1.9
+    V = synth.vol(L)
+    g = B.geom_create(L)
+    Uc = torch.from_numpy(synth.su2_matrices(synth.smooth_su2_cd(L, synth.seed_for(5, 20)))).cuda()
+    U64 = B.su2_alloc_field(g, B.FIELD_GAUGE)
+    B.su2_gauge_import(g, Uc, U64)
+    U32 = B.su2_alloc_field(g, B.FIELD_GAUGE, B.F32)
+    B.su2_gauge_import(g, Uc, U32, B.F32)
+    del Uc
+    psic = torch.view_as_complex(torch.randn((V, 4, 2, 2), dtype=torch.float64, device="cuda",
+                                             generator=torch.Generator(device="cuda").manual_seed(synth.seed_for(5, 21))))
+    out = {}
+    for p, pname, rb, U in ((B.F64, "f64", 8, U64), (B.F32, "f32", 4, U32)):
+        A = B.su2_alloc_field(g, B.FIELD_CLOVER, p)
+        B.su2_clover_build(g, kappa, csw, U64, A, p)
+        src, dst = B.su2_alloc_field(g, B.FIELD_SPINOR, p), B.su2_alloc_field(g, B.FIELD_SPINOR, p)
+        B.su2_spinor_import(g, psic, src, p)
+        ms = time_calls(torch, lambda: B.su2_dw_apply(g, kappa, U, A, src, dst, False, p), 10)
+        gb = 80 * rb * V / (ms * 1e-3) / 1e9
+        out["next4_su2_dw_%s" % pname] = {"ms": round(ms, 4), "GFLOP/s": round(864 * V / ms / 1e6, 1), "GB/s": round(gb, 1),
+                                          "frac_measured_peak": round(gb / peak, 4), "lattice": "x".join(str(v) for v in L),
+                                          "model": "80 reals/site compulsory, 864 flop/site"}
+        del A, src, dst
+    B.geom_destroy(g)
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_config2(torch, B, synth, peak):
