@@ -346,3 +346,34 @@ def test_cg_eo_multi_tile(mode, mixed):
     assert np.linalg.norm(got - xo) / np.linalg.norm(xo) <= 200 * (rt + rt_o)
     assert np.all(got[~interior(L, bc)] == 0)
     lat.close()
+
+
+def test_concurrent_launches_on_one_geometry():
+    """The pipeline kernel's tile counters come from a pool owned by the geometry (one pair per launch in flight): D on
+    two CUDA streams at the same time, on the same geometry and gauge field, must give what two launches one after the
+    other give (bit for bit: the arithmetic per tile does not depend on which CTA draws it)."""
+    L, kappa, csw = (16, 16, 16, 16), 0.137, 1.9
+    dev = torch.device("cuda", torch.cuda.current_device())
+    lat = Lattice(L)
+    lat.set_gauge(synth.smooth_gauge_torch(L, 401, dev))
+    lat.build_clover(kappa, csw)
+    srcs = [lat.spinor(synth.gaussian_spinor_torch(L, 402 + i, dev)) for i in range(2)]
+    ref = []
+    for s in srcs:
+        d = lat.alloc(B.FIELD_SPINOR)
+        B.dw_apply(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], s, d)
+        ref.append(d)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for rep in range(20):
+        outs = [lat.alloc(B.FIELD_SPINOR) for _ in range(2)]
+        for o in outs:
+            o.fill_(0x7F)
+        torch.cuda.synchronize()
+        for i in range(2):
+            for _ in range(3):   # three launches per stream, interleaved with the other stream's
+                B.dw_apply(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], srcs[i], outs[i], stream=streams[i].cuda_stream)
+        torch.cuda.synchronize()
+        for i in range(2):
+            assert torch.equal(outs[i], ref[i]), rep
+    lat.close()
