@@ -377,3 +377,53 @@ def test_concurrent_launches_on_one_geometry():
         for i in range(2):
             assert torch.equal(outs[i], ref[i]), rep
     lat.close()
+
+
+@pytest.mark.parametrize("prec", [B.F64, B.F32])
+def test_full_grid_launches_repeat_bit_for_bit(prec):
+    """Race evidence without a sanitizer, at a size where all 148 CTAs run and draw their tiles from the counter in a
+    different order every launch (32^4 = 4096 tiles): D, D^+, both passes of D^ and the staged clover builder, 25
+    launches each into a poisoned output, must reproduce the first launch bit for bit.  (The half-lattice kernel's
+    buffer-release race of round 2 showed up exactly like this: a few tiles per launch, different ones every run.)"""
+    L, kappa, csw = (32, 32, 32, 32), 0.137, 1.9
+    dev = torch.device("cuda", torch.cuda.current_device())
+    lat = Lattice(L)
+    lat.set_gauge(synth.smooth_gauge_torch(L, 501, dev), precs=(prec,))
+    lat.build_clover(kappa, csw, precs=(prec,), inverse=True)
+    assert B.geom_info(lat.g)[0] == [4, 4, 4, 4]
+    U, A, Ai = lat.U[(prec, 18)], lat.A[prec], lat.Ainv[prec]
+    src = lat.spinor(synth.gaussian_spinor_torch(L, 502, dev), prec)
+    tmp = lat.alloc(B.FIELD_SPINOR, prec)
+    A2, Ai2 = lat.alloc(B.FIELD_CLOVER, prec), lat.alloc(B.FIELD_CLOVER, prec)
+
+    def clover(out):
+        A2.fill_(0x7F)
+        B.clover_build(lat.g, kappa, csw, lat.U[(B.F64, 18)], A2, Ai2 if prec == B.F64 else None, 18, prec)
+        return A2
+
+    def stencil(fn):
+        def run(out):
+            fn(out)
+            return out
+        return run
+
+    ops = {
+        "D": stencil(lambda out: B.dw_apply(lat.g, kappa, U, A, src, out, prec, 18)),
+        "D^+": stencil(lambda out: B.dwdag_apply(lat.g, kappa, U, A, src, out, prec, 18)),
+        "D^": stencil(lambda out: B.dw_eo_apply(lat.g, kappa, U, A, Ai, src, out, tmp, False, prec, 18)),
+        "Csw": clover,
+    }
+    for name, op in ops.items():
+        first = None
+        for rep in range(25):
+            out = lat.alloc(B.FIELD_SPINOR, prec)
+            out.fill_(0x7F)
+            res = op(out)
+            torch.cuda.synchronize()
+            if first is None:
+                first = res.clone()
+            else:
+                assert torch.equal(res, first), (name, rep)
+    if prec == B.F64:   # (fp32 blocks with an inverse come from the one-thread-per-site kernel: equal up to one rounding)
+        assert torch.equal(A2, A) and torch.equal(Ai2, Ai)
+    lat.close()
