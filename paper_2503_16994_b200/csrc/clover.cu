@@ -10,7 +10,9 @@
 // (R14); the result is rounded once to the requested precision.
 #include <stdlib.h>
 
+#include <algorithm>
 #include <mutex>
+#include <utility>
 #include <vector>
 
 #include "kernels.cuh"
@@ -395,10 +397,10 @@ __host__ __device__ inline StageBox make_box(int mu, int nu, bool is_nu) {
 // 32-bit word per link, built on the host at first use (ct_table_upload):
 //   bits 0-9 index r in the staged array, 10-16 neighbour tile (index into sNb), 17-23 checkerboard index j in that
 //   tile, 24 parity, 25 box (0: U_mu, 1: U_nu), 26-28 time offset from the slab's first slice plus one; ~0 = none
-constexpr int CT_NIT = 3;   // 374 <= 3 * 128
 #ifndef CT_REG
-#define CT_REG 1            // of which the first goes through registers (see ct_table_build)
+#define CT_REG 2            // table slots (of 128 links) that go through registers (see ct_table_build)
 #endif
+constexpr int CT_NIT = CT_REG + 2;   // two more slots for cp.async
 __device__ uint32_t ct_table[2][6][CT_NIT * CT_THREADS];
 
 // plane number pl = 2 * step + half of the kernel's loop -> (mu, nu)
@@ -416,6 +418,10 @@ static void ct_table_build(uint32_t* tab) {
       const StageBox ba = make_box(mu, nu, false), bb = make_box(mu, nu, true);
       uint32_t* t = tab + (size_t)(s * 6 + pl) * CT_NIT * CT_THREADS;
       for (int i = 0; i < CT_NIT * CT_THREADS; i++) t[i] = ~0u;
+      // fringe links whose x1 and x2 coordinates lie inside the slab come in whole runs of 8 consecutive j
+      // (128 bytes per row): time slices next to the slab, x3 layers, their corners.  Sorted by address they fill the
+      // first CT_REG slots, which go through registers; everything else (and what does not fit) is copied by cp.async.
+      std::vector<std::pair<uint32_t, uint32_t>> runs;   // (sort key, word)
       int n = CT_REG * CT_THREADS;
       for (int idx = 0; idx < ba.n + bb.n; idx++) {
         const bool isb = idx >= ba.n;
@@ -427,11 +433,10 @@ static void ct_table_build(uint32_t* tab) {
         cc[3] = q / b.E[2];
         const int r = (isb ? ba.size : 0) + cc[1] + b.S[2] * cc[2] + b.S[3] * cc[3] + b.S[0] * cc[0];
         int nb = 0;
-        bool own = true, column = true;   // column: above or below the slab in time
+        bool own = true;
         for (int d = 3; d >= 0; d--) {
           rel[d] = cc[d] - b.o[d];   // coordinate relative to the slab
           own = own && rel[d] >= 0 && rel[d] < (d == 3 ? 2 : 4);
-          column = column && (d == 3 || (rel[d] >= 0 && rel[d] < 4));
           l[d] = rel[d] + (d == 3 ? 2 * s : 0);
           nb = nb * 3 + (l[d] < 0 ? 0 : (l[d] >= 4 ? 2 : 1));
           l[d] &= 3;
@@ -441,25 +446,34 @@ static void ct_table_build(uint32_t* tab) {
         const int p = (l[0] + l[1] + l[2] + l[3]) & 1;
         const uint32_t word = (uint32_t)r | (uint32_t)nb << 10 | (uint32_t)j << 17 | (uint32_t)p << 24 | (uint32_t)isb << 25 |
                               (uint32_t)(rel[3] + 1) << 26;
-        // the two full time slices next to the slab in box A of a (k, 4) plane: 32 consecutive j per parity and slice,
-        // i.e. whole 512-byte runs -- slot 0, which goes through registers
-        if (CT_REG == 1 && !isb && nu == 3 && column) {
-          t[64 * (rel[3] > 0) + 32 * p + (j & 31)] = word;
+        if (rel[0] >= 0 && rel[0] < 4 && rel[1] >= 0 && rel[1] < 4) {
+          runs.push_back(std::make_pair((uint32_t)isb << 16 | (uint32_t)nb << 8 | (uint32_t)p << 7 | (uint32_t)j, word));
           continue;
         }
-        if (n >= CT_NIT * CT_THREADS) abort();   // cannot happen: at most 374 fringe links, 246 without the slices
+        if (n >= CT_NIT * CT_THREADS) abort();   // cannot happen (see the counts in DESIGN.md)
         t[n++] = word;
+      }
+      std::sort(runs.begin(), runs.end());
+      for (size_t i = 0; i < runs.size(); i++) {
+        if (i < (size_t)CT_REG * CT_THREADS) t[i] = runs[i].second;
+        else {
+          if (n >= CT_NIT * CT_THREADS) abort();
+          t[n++] = runs[i].second;
+        }
       }
     }
 }
 
-// Copies the links of both boxes of a plane into sU[k][r] (box A = U_mu from 0, box B = U_nu from ba.size): every
-// thread takes up to CT_NIT links and issues nine 16-byte cp.async for each -- no registers in flight, one round trip
-// to L2 per plane.  This is what bounds the kernel: a 16-byte cp.async lands as one shared-memory wavefront per LANE
-// (32 per instruction), 2.4 G wavefronts at 48^3 x 96 = 8.4 ms of the load/store pipe, next to 0.94 G for the reads
-// of the arithmetic.  Loading into registers and storing (LDG.128 + STS.128, 8 wavefronts per instruction pair) was
-// measured too: its round trips are exposed -- two CTAs of four warps cannot cover them -- and it came out slower
-// (profiles/r02_notes.md, section 12).  RECON 12: the third row is rebuilt once the copies have landed.
+// Copies the links of both boxes of a plane into sU[k][r] (box A = U_mu from 0, box B = U_nu from ba.size).
+// A 16-byte cp.async costs one shared-memory wavefront per LANE (32 per instruction; with every link staged that way
+// the copies alone were 2.4 G wavefronts = 8.4 ms of the load/store pipe at 48^3 x 96, next to 0.94 G for the reads of
+// the arithmetic), a 16-byte load into a register plus a 16-byte store costs a quarter of that but holds registers and
+// exposes its round trip.  So: what a warp can load in whole 128-byte lines goes through registers, all of it in
+// flight together -- the thread's own two links, and CT_REG table slots of fringe links that come in runs of eight
+// consecutive j -- and the scattered rest of the fringe (x1 and x2 faces: 16- and 32-byte pieces) is copied by
+// cp.async while those loads are under way.  Scattered links through registers, or more than one batch of register
+// loads, were measured slower (profiles/r02_notes.md, section 12).  RECON 12: the third row is rebuilt in registers,
+// or in shared memory once the copies have landed.
 template <int RECON>
 __device__ __forceinline__ void recon_row3(double2 (&v)[9]) {
   if (RECON == 12) {
@@ -553,7 +567,7 @@ __device__ __noinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, c
 #pragma unroll 1
   for (int it = 0; it < CT_NIT; it++) {
     const uint32_t ent = __ldg(tb + threadIdx.x + it * CT_THREADS);
-    if (ent == ~0u) break;
+    if (ent == ~0u) continue;   // slots are filled from the front, but not to the end
     const int t = sNb[(ent >> 10) & 127], j = (ent >> 17) & 127, p = (ent >> 24) & 1;
     const int dir = (ent >> 25) & 1 ? nu : mu;
     const int x3 = t0 + (int)((ent >> 26) & 7) - 1;
