@@ -447,7 +447,9 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
     wsc = B.alloc_field(g, B.FIELD_WORKSPACE)
     ms = time_calls(torch, lambda: B.correlator_ps(g, src, nrhs, wsc, L[3]), 3)
     rows["next2_correlator_ps_12cols_f64"] = {"ms": round(ms, 3), "GB/s": gbs(24 * nrhs, 8, ms),
-                                              "frac_measured_peak": round(gbs(24 * nrhs, 8, ms) / peak, 4)}
+                                              "frac_measured_peak": round(gbs(24 * nrhs, 8, ms) / peak, 4),
+                                              "note": "a pure read stream: the peak it is divided by was measured with a "
+                                                      "copy (reads + writes), which a read-only kernel can exceed"}
     del src, dst, wsc
     # NEXT-3: the same lattice as ONE time slab -- pack, face exchange with itself (the periodic
     # wrap) on a side stream, stencil without the two face hops, face kernel.  What a rank of a decomposed lattice
