@@ -441,8 +441,10 @@ def run_rows(torch, B, synth, S, args, prec, recon, peak):
     rows["next1_dw_multi_12rhs_f64"] = {
         "ms": round(ms, 3), "ms_per_rhs": round(ms / nrhs, 4), "GFLOP/s": round(nrhs * FLOP_DW * V / ms / 1e6, 1),
         "GB/s_model": gbs(reals_multi, 8, ms), "model": "%d reals/site for 12 columns (links + clover once)" % reals_multi,
-        "note": "no gain over 12 single applications yet: with the links served by L2 the pipeline is bound by its "
-                "arithmetic warps (about 2.6 ms per right-hand side)"}
+        "vs_single_application": round(ms / nrhs / dw["dw_f64_recon%d" % recon]["ms"], 3),
+        "note": "a tile's 12 columns are shared out over 4 work units drawn one after the other (3 columns each), so its "
+                "links and clover blocks come from HBM about once; what is left is the arithmetic warps' time per tile "
+                "with every operand in L2 (8.5 us against 10.4 us from HBM, profiles/r02_notes.md section 11)"}
     # NEXT-2: pseudoscalar two-point function of 12 columns (a pure reduction: 12 x 24 reals per site read once)
     wsc = B.alloc_field(g, B.FIELD_WORKSPACE)
     ms = time_calls(torch, lambda: B.correlator_ps(g, src, nrhs, wsc, L[3]), 3)

@@ -402,9 +402,9 @@ __device__ __forceinline__ int tq_pop(PipeBars* bars, const int kt, const int la
   if (lane == 0) mbar_arrive(&bars->tq_empty[q]);
   return tile;
 }
-__device__ __forceinline__ int next_tile(const Geom& g, unsigned int* sched, const int tile) {
+__device__ __forceinline__ int next_tile(const int nunits, unsigned int* sched, const int tile) {
   const int n = sched ? (int)(gridDim.x + atomicAdd(sched, 1u)) : tile + (int)gridDim.x;
-  return n < g.ntiles ? n : -1;
+  return n < nunits ? n : -1;
 }
 
 struct RingPos {
@@ -574,6 +574,11 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   __syncthreads();
   double nrm = 0.0;
   const int nrhs = a.nrhs > 1 ? a.nrhs : 1;
+  // work unit u = (tile u / nsplit, right-hand sides [(u % nsplit) nper, + nper)): units of one tile are drawn one after
+  // the other, so the CTAs that share a tile's links and clover blocks read them at about the same time (L2)
+  const int nsplit = (a.nrhs > 1 && a.nsplit > 1) ? a.nsplit : 1;
+  const int nper = nrhs / nsplit;
+  const int NUNITS = g.ntiles * nsplit;
   const uint32_t stage_bytes = (uint32_t)(NCU * TV * sizeof(T2<T>));
   const uint32_t sp_bytes = (uint32_t)(12 * TV * sizeof(T2<T>));
 
@@ -585,20 +590,23 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         const uint64_t pol_once = policy_evict_first();
         RingPos rp = {0, 0u};
         int k = 0, kt = 0;
-        int tile = blockIdx.x;   // the host keeps gridDim.x <= ntiles
-        int tile_after = next_tile(g, a.sched, tile);
+        int tile = blockIdx.x;   // a work unit; the host keeps gridDim.x <= the number of units
+        int tile_after = next_tile(NUNITS, a.sched, tile);
         tq_push(bars, kt++, tile);
         while (tile >= 0) {
         // the halo warps run half a tile ahead of the arithmetic warps: they get the next index (or the end marker) now,
         // and the draw for the tile after that is in flight while this tile is streamed
         tq_push(bars, kt++, tile_after);
-        const int tile_after2 = tile_after >= 0 ? next_tile(g, a.sched, tile_after) : -1;
-        for (int rhs = 0; rhs < nrhs; rhs++, k++) {   // all right-hand sides of a tile back to back: links and clover
+        const int tile_after2 = tile_after >= 0 ? next_tile(NUNITS, a.sched, tile_after) : -1;
+        const int unit = tile, r0 = (unit % nsplit) * nper;
+        {
+        const int tile = unit / nsplit;
+        for (int rhs = r0; rhs < r0 + nper; rhs++, k++) {   // the unit's right-hand sides back to back: links and clover
                                                        // blocks of the 2nd..nth pass come out of L2
           if (k == 0) {
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
-              bulk_g2s(sp + (p * 12) * TV, a.in + field_offset(g, 12, p, tile, 0, 0), sp_bytes, &bars->full_sp);
+              bulk_g2s(sp + (p * 12) * TV, a.in + rhs * a.rhs_stride + field_offset(g, 12, p, tile, 0, 0), sp_bytes, &bars->full_sp);
           }
 #pragma unroll 1
           for (int st = 0; st < 4 + NSTC; st++) {   // stage order: L0 L1 [A+] L2 L3 [A-]  (consumer loop below)
@@ -615,7 +623,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
               if (mu >= 0)
                 bulk_g2s(dst + (p * NCU) * TV, a.U + field_offset(g, 4 * NCU, p, tile, mu * NCU, 0), stage_bytes,
                          &bars->full[rp.slot]);
-              else if (rhs + 1 < nrhs)
+              else if (rhs + 1 < r0 + nper)
                 bulk_g2s(dst + (p * NCU) * TV, a.A + field_offset(g, 36, p, tile, cs * NCU, 0), stage_bytes,
                          &bars->full[rp.slot]);
               else   // clover blocks are read for the last time: evict-first keeps them from displacing spinors and links in L2
@@ -625,7 +633,10 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             rp.advance(nslot);
           }
           int next = tile, nr = rhs + 1;
-          if (nr == nrhs) { nr = 0; next = tile_after; }
+          if (nr == r0 + nper) {
+            next = tile_after >= 0 ? tile_after / nsplit : -1;
+            nr = tile_after >= 0 ? (tile_after % nsplit) * nper : 0;
+          }
           if (next >= 0) {  // spinor of the next pass: its buffer is released after this pass's hops
             mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
             mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
@@ -633,6 +644,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
               bulk_g2s(sp + (p * 12) * TV, a.in + nr * a.rhs_stride + field_offset(g, 12, p, next, 0, 0), sp_bytes,
                        &bars->full_sp);
           }
+        }
         }
         tile = tile_after;
         tile_after = tile_after2;
@@ -643,9 +655,10 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       const int lt = tid - (PIPE_CONS_WARPS + 1) * 32;
       RingPos hp = {0, 0u};   // halo buffer ring
       for (int kt = 0;; kt++) {
-      const int tile = tq_pop(bars, kt, lane);
-      if (tile < 0) break;
-      for (int rhs = 0; rhs < nrhs; rhs++) {
+      const int unit = tq_pop(bars, kt, lane);
+      if (unit < 0) break;
+      const int tile = unit / nsplit, r0 = (unit % nsplit) * nper;
+      for (int rhs = r0; rhs < r0 + nper; rhs++) {
         const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
         const T2<T>* in_r = a.in + rhs * a.rhs_stride;
         for (int mu = 0; mu < 4; mu++) {
@@ -673,9 +686,10 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     RingPos hp = {0, 0u};
     int k = 0;
     for (int kt = 0;; kt++) {
-    const int tile = tq_pop(bars, kt, lane);
-    if (tile < 0) break;
-    for (int rhs = 0; rhs < nrhs; rhs++, k++) {
+    const int unit = tq_pop(bars, kt, lane);
+    if (unit < 0) break;
+    const int tile = unit / nsplit, r0 = (unit % nsplit) * nper;
+    for (int rhs = r0; rhs < r0 + nper; rhs++, k++) {
       const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
       const int x3 = __ldg(tab + 8) + l[3];
       const bool live = !(nonper && frozen_slice(g, x3));
@@ -915,6 +929,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     mbar_fence_init();
   }
   __syncthreads();
+  const int NUNITS = g.ntiles;
   const uint32_t link_bytes = (uint32_t)(NCU * TV * sizeof(T2<T>));
   const uint32_t clv_bytes = (uint32_t)(HALF_CLV_ROWS * TV * sizeof(T2<T>));
   const uint32_t sp_bytes = (uint32_t)(12 * TV * sizeof(T2<T>));
@@ -928,7 +943,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         RingPos rp = {0, 0u};
         int k = 0, kt = 0;
         int tile = blockIdx.x;
-        int tile_after = next_tile(g, a.sched, tile);
+        int tile_after = next_tile(NUNITS, a.sched, tile);
         tq_push(bars, kt++, tile);
         auto load_spinors = [&](const int t) {
           mbar_arrive_expect_tx(&bars->full_sp, (SELF ? 2 : 1) * sp_bytes);
@@ -938,7 +953,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         load_spinors(tile);
         while (tile >= 0) {
           tq_push(bars, kt++, tile_after);
-          const int tile_after2 = tile_after >= 0 ? next_tile(g, a.sched, tile_after) : -1;
+          const int tile_after2 = tile_after >= 0 ? next_tile(NUNITS, a.sched, tile_after) : -1;
 #pragma unroll 1
           for (int st = 0; st < 4 + NSTC; st++) {   // L0 L1 L2 L3 C0 C1 C2 C3
             mbar_wait_relaxed(&bars->empty[rp.slot], rp.ph ^ 1u);
@@ -1274,7 +1289,23 @@ static cudaError_t launch_pipe(const Geom& g, const DwArgs<T>& a, const PipeCfg&
   if (e != cudaSuccess) return e;
   DwArgs<T> b = a;
   b.sched = sched_slot(g);
-  dw_pipe_kernel<T, RECON, DIAG><<<c.grid, PIPE_THREADS, c.smem, s>>>(g, b, c.nslot);
+  // several right-hand sides: every tile becomes nsplit work units of nrhs / nsplit columns each.  148 CTAs each on a
+  // tile of its own keep 65 MB of links and clover blocks in flight between the passes, more than L2 holds next to the
+  // spinor streams (measured: 12.5 GB of DRAM reads per column, 0 % gain); with the columns of a tile shared out over
+  // neighbouring CTAs the set shrinks by nsplit and a tile's links come from DRAM once.
+  int grid = c.grid;
+  b.nsplit = 1;
+  if (a.nrhs > 1) {
+    int want = env_int("LQCD_NSPLIT", 4);
+    if (want < 1) want = 1;
+    while (want > 1 && a.nrhs % want != 0) want--;
+    b.nsplit = want;
+    const long long units = (long long)g.ntiles * want;
+    grid = g.sm_count;
+    if (g_pipe_grid > 0 && g_pipe_grid < grid) grid = g_pipe_grid;
+    if (grid > units) grid = (int)units;
+  }
+  dw_pipe_kernel<T, RECON, DIAG><<<grid, PIPE_THREADS, c.smem, s>>>(g, b, c.nslot);
   count_launch();
   return cudaGetLastError();
 }

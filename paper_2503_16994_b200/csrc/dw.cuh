@@ -29,6 +29,7 @@ struct DwArgs {
   unsigned int* sched;                 // pipeline kernel: {next tile, finished CTAs} of its tile scheduler (NULL: static)
   int nrhs;                            // > 1: in / out are arrays of nrhs spinor fields rhs_stride complex numbers apart
   long long rhs_stride;                //      (several right-hand sides share the links and the clover term)
+  int nsplit;                          //      pipeline kernel: a tile's right-hand sides are shared out over nsplit work units (set by launch_pipe)
 };
 
 // number of per-CTA partial sums an EPI_*_NORM launch with these arguments writes to DwArgs::partial

@@ -105,10 +105,14 @@ def test_plan_and_option_errors():
 
 @pytest.mark.parametrize("mode", ["pipe", "stream"], indirect=True)
 @pytest.mark.parametrize("prec", [B.F64, B.F32])
-def test_dw_apply_multi(mode, prec):
+@pytest.mark.parametrize("nrhs,grid", [(3, 0), (8, 0), (8, 5)])
+def test_dw_apply_multi(mode, prec, nrhs, grid):
     """several right-hand sides in one pass share the links and clover blocks; the result
-    is the oracle's for every column and bit-identical to separate lqcd_dw_apply calls."""
-    L, bc, theta, kappa, csw, nrhs = (8, 4, 8, 12), B.BC_OPEN, (0.5, 0.5, 0.5, 0.0), 0.137, 1.9, 3
+    is the oracle's for every column and bit-identical to separate lqcd_dw_apply calls.  The pipeline kernel shares a
+    tile's columns out over up to four work units (3 columns: three units of one; 8: four units of two); with a grid
+    of 5 CTAs every CTA walks many units."""
+    L, bc, theta, kappa, csw = (8, 4, 8, 12), B.BC_OPEN, (0.5, 0.5, 0.5, 0.0), 0.137, 1.9
+    B.set_option("pipe_grid", str(grid))
     U = synth.smooth_gauge(L, 81)
     A = oracle.clover_blocks(L, U, kappa, csw, bc=bc)
     psis = [synth.gaussian_spinor(L, 82 + n) for n in range(nrhs)]
@@ -134,6 +138,7 @@ def test_dw_apply_multi(mode, prec):
             fn(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src[n * fb:(n + 1) * fb], single, prec)
             torch.cuda.synchronize()
             assert torch.equal(single, dst[n * fb:(n + 1) * fb])
+    B.set_option("pipe_grid", "0")
     with pytest.raises(B.LqcdError):   # overlapping arrays
         B.dw_apply_multi(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], src, src[fb:], 2, prec)
     lat.close()
