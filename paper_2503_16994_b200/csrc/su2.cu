@@ -22,10 +22,15 @@ struct Site2 {
 __device__ __forceinline__ bool site2_from_thread(const Geom& g, Site2& s) {
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 2 * g.Vh) return false;
-  s.p = (int)(idx / g.Vh);
-  const long long rem = idx - (long long)s.p * g.Vh;
-  s.tile = (int)(rem / g.TV);
-  s.j = (int)(rem - (long long)s.tile * g.TV);
+  // a CTA (128 threads) takes runs of JC = min(64, TV) consecutive checkerboard indices of BOTH parities of a tile
+  // (4^4 tiles: a 4x4x4x2 slab), so that most neighbours of a site are fetched by the same CTA and hit in L1
+  const int JC = g.TV < 64 ? g.TV : 64;
+  const long long unit = idx / (2 * JC);
+  const int r = (int)(idx - unit * (2 * JC));
+  const int cpt = g.TV / JC;   // runs per tile
+  s.tile = (int)(unit / cpt);
+  s.p = r / JC;
+  s.j = (int)(unit - (long long)s.tile * cpt) * JC + (r - s.p * JC);
   local_coords(g, s.j, s.p, s.l);
   s.x3 = __ldg(g.tile_tab + (size_t)s.tile * TILE_TAB + 8) + s.l[3];
   return true;
@@ -304,8 +309,12 @@ __device__ __forceinline__ void hop_both(const Geom& g, const Su2Args& a, const 
 }
 
 // out = A in - kappa H in (or its gamma5 conjugate); A = NULL means csw = 0
+// A latency-bound gather kernel: resident warps are what counts.  Measured at 48^3 x 96 (one gpurun call each): fp64
+// 140 registers / 3 CTAs per SM 1.74 ms, 128 / 4 CTAs 1.46 ms, 96 / 5 CTAs (spills) 1.67 ms; fp32 80 registers / 6 CTAs
+// 0.91 ms, 64 / 8 CTAs 0.84 ms.
+enum { SU2_MINB64 = 4, SU2_MINB32 = 8 };
 template <typename T>
-__global__ void __launch_bounds__(SU2_THREADS) su2_dw_kernel(const Geom g, const Su2Args a, const T2<T>* __restrict__ U,
+__global__ void __launch_bounds__(SU2_THREADS, sizeof(T) == 8 ? SU2_MINB64 : SU2_MINB32) su2_dw_kernel(const Geom g, const Su2Args a, const T2<T>* __restrict__ U,
                                                              const T2<T>* __restrict__ A, const T2<T>* __restrict__ in, T2<T>* out) {
   Site2 s;
   if (!site2_from_thread(g, s)) return;
