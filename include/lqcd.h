@@ -158,6 +158,20 @@ lqcd_status lqcd_spinor_dot(const lqcd_geom* g, const void* u, const void* v, in
 lqcd_status lqcd_correlator_ps(const lqcd_geom* g, const void* columns, int ncol, lqcd_prec prec, void* workspace,
                                double* C_host, void* stream);
 
+/* The same for callers that cannot allocate device memory or provide a
+ * workspace -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The scratch
+ * (ntiles * tile extent in time + L4 doubles) is a static array of LQCD_CORRELATOR_STATIC_MAX_DOUBLES doubles
+ * (1.5 MiB) in the device memory of every GPU that loads the library, held until the process exits; the call itself
+ * makes no cudaMalloc / cudaFree and calls no allocating library routine.  Same kernels as lqcd_correlator_ps: the
+ * result is bit-identical.  columns: DEVICE, ncol internal spinor fields back to back; C_host: HOST, L4 doubles, valid
+ * on return (the call synchronises the stream).  Errors: LQCD_EINVAL for NULL / bad enum / ncol outside 1..4096, and
+ * for a lattice whose scratch does not fit (e.g. 64^3 x 128; 48^3 x 96 fits) -- use lqcd_correlator_ps then.
+ * All calls on a device share the array (nothing in it needs clearing: every element read is written earlier in the
+ * same call), so calls that overlap on the GPU -- other streams, other host threads -- race: serialise them. */
+#define LQCD_CORRELATOR_STATIC_MAX_DOUBLES 196608
+lqcd_status lqcd_correlator_ps_static(const lqcd_geom* g, const void* columns, int ncol, lqcd_prec prec, double* C_host,
+                                      void* stream);
+
 /* End-to-end call over HOST buffers in the canonical layout (SURVEY.md 8(b), 8(d) "e2e"; Csw! then
  * Dw! on a configuration that lives on the host).  U_canon_host [V][4][3][3], in_canon_host / out_canon_host [V][4][3],
  * complex fp64, HOST memory (pinned memory makes the copies asynchronous; pageable memory works).  The gauge field is

@@ -24,7 +24,7 @@ EXPORTS = [
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
     "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_host_cache_release", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
-    "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
+    "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_correlator_ps_static", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
     "lqcd_clover_build_slab", "lqcd_cg_solve_slab",
     "lqcd_su2_field_bytes", "lqcd_su2_gauge_import", "lqcd_su2_gauge_export", "lqcd_su2_spinor_import",
     "lqcd_su2_spinor_export", "lqcd_su2_clover_build", "lqcd_su2_clover_export", "lqcd_su2_dw_apply", "lqcd_su2_cg_solve",
@@ -328,6 +328,17 @@ def correlator_ps(g, columns, ncol, workspace, L4, prec=F64, stream=None):
     """C(x4) = sum_xvec sum_{columns, spin, colour} |S|^2 as a list of L4 floats."""
     C = (ctypes.c_double * int(L4))()
     _check(lib().lqcd_correlator_ps(g, _ptr(columns), int(ncol), prec, _ptr(workspace), C, _stream(stream)))
+    return list(C)
+
+
+CORRELATOR_STATIC_MAX_DOUBLES = 196608   # include/lqcd.h: LQCD_CORRELATOR_STATIC_MAX_DOUBLES
+
+
+def correlator_ps_static(g, columns, ncol, L4, prec=F64, stream=None):
+    """lqcd_correlator_ps without a workspace and without any allocation: the scratch is a static device array of the
+    library (lattices up to ntiles * b4 + L4 <= CORRELATOR_STATIC_MAX_DOUBLES; calls must not overlap on the GPU)."""
+    C = (ctypes.c_double * int(L4))()
+    _check(lib().lqcd_correlator_ps_static(g, _ptr(columns), int(ncol), prec, C, _stream(stream)))
     return list(C)
 
 

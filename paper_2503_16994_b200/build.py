@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "liblqcd_b200.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "blas.cu", "cg.cu", "clover.cu", "dw.cu", "layout.cu", "slab.cu", "su2.cu"]
+SOURCES = ["api.cu", "blas.cu", "cg.cu", "clover.cu", "dw.cu", "layout.cu", "noalloc.cu", "slab.cu", "su2.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
