@@ -292,6 +292,7 @@ lqcd_status lqcd_geom_create(const lqcd_geom_desc* desc, lqcd_geom** out) {
           tab[(size_t)t * TILE_TAB + 2 * mu + d] = tile_linear(g, Tn[0], Tn[1], Tn[2], Tn[3]);
         }
       tab[(size_t)t * TILE_TAB + 8] = Tc[3] * g.b[3];
+      for (int i = 0; i < 3; i++) tab[(size_t)t * TILE_TAB + 9 + i] = Tc[i] * g.b[i];   // spatial origin of the tile
     }
     int* dtab = nullptr;
     if (!cuda_ok(cudaMalloc(&dtab, tab.size() * sizeof(int)), "cudaMalloc(tile table)")) { free(h); return LQCD_ENOMEM; }

@@ -342,6 +342,7 @@ static cudaError_t clover_launch(const CloverCtx& c, const CloverParm& cp, void*
 // (x1 fastest, or the parity-split layout of the global fields, cannot achieve that for offsets along x1).
 
 constexpr int CT_THREADS = 128;
+constexpr int CT_TV = 128;       // sites of one parity in a 4^4 tile: compile-time, so that row offsets are immediates
 constexpr int CT_NR = 632;        // staged links per plane (largest: plane (1,4), 330 + 300 with padding)
 constexpr size_t CT_SMEM = (size_t)9 * CT_NR * sizeof(double2) + (size_t)18 * CT_THREADS * sizeof(double) + 81 * sizeof(int) + 12;
 
@@ -494,9 +495,9 @@ __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, con
   constexpr int NCU = RECON == 12 ? 6 : 9;
   double2 va[9], vb[9];
 #pragma unroll
-  for (int k = 0; k < NCU; k++) va[k] = __ldg(own + (size_t)(mu * NCU + k) * g.TV);
+  for (int k = 0; k < NCU; k++) va[k] = __ldg(own + (size_t)(mu * NCU + k) * CT_TV);
 #pragma unroll
-  for (int k = 0; k < NCU; k++) vb[k] = __ldg(own + (size_t)(nu * NCU + k) * g.TV);
+  for (int k = 0; k < NCU; k++) vb[k] = __ldg(own + (size_t)(nu * NCU + k) * CT_TV);
   uint32_t ent[CT_NIT];
 #pragma unroll
   for (int it = 0; it < CT_NIT; it++) ent[it] = __ldg(tb + threadIdx.x + it * CT_THREADS);
@@ -511,10 +512,10 @@ __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, con
     double2* dst = sU + (en & 1023);
     if (it < CT_REG) {
 #pragma unroll
-      for (int k = 0; k < NCU; k++) vf[it < CT_REG ? it : 0][k] = __ldg(src + (size_t)k * g.TV);
+      for (int k = 0; k < NCU; k++) vf[it < CT_REG ? it : 0][k] = __ldg(src + (size_t)k * CT_TV);
     } else {
 #pragma unroll
-      for (int k = 0; k < NCU; k++) cp_async_16(dst + k * CT_NR, src + (size_t)k * g.TV);
+      for (int k = 0; k < NCU; k++) cp_async_16(dst + k * CT_NR, src + (size_t)k * CT_TV);
     }
   }
   recon_row3<RECON>(va);
@@ -550,7 +551,7 @@ __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, con
 // The same for the planes of a slab that reach past the lattice in time: SF, the slice x4 = L4 is the boundary
 // field W' (D7); LQCD_BC_SLAB, slices outside the slab come from the gauge halos.  One link at a time.
 template <int RECON>
-__device__ __noinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, const int* sNb, const uint32_t* tb, int mu, int nu, int t0,
+__device__ __forceinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, const int* sNb, const uint32_t* tb, int mu, int nu, int t0,
                                               const double2* own, int ra, int rb) {
   const Geom& g = c.g;
   constexpr int NCU = RECON == 12 ? 6 : 9;
@@ -558,7 +559,7 @@ __device__ __noinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, c
   for (int w = 0; w < 2; w++) {   // the thread's own two links (always inside the lattice)
     double2 v[9];
 #pragma unroll
-    for (int k = 0; k < NCU; k++) v[k] = __ldg(own + (size_t)((w ? nu : mu) * NCU + k) * g.TV);
+    for (int k = 0; k < NCU; k++) v[k] = __ldg(own + (size_t)((w ? nu : mu) * NCU + k) * CT_TV);
     recon_row3<RECON>(v);
 #pragma unroll
     for (int k = 0; k < 9; k++) sU[k * CT_NR + (w ? rb : ra)] = v[k];
@@ -586,10 +587,10 @@ __device__ __noinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, c
         }
       }
     } else if (g.bc == LQCD_BC_SLAB && (x3 < 0 || x3 >= g.L[3])) {
-      int Tc[4], l[4];
-      tile_coords(g, t, Tc);
+      int l[4];
       local_coords(g, j, p, l);
-      const int n = (Tc[0] * 4 + l[0]) + g.L[0] * ((Tc[1] * 4 + l[1]) + g.L[1] * (Tc[2] * 4 + l[2]));
+      const int* org = g.tile_tab + (size_t)t * TILE_TAB + 9;   // space coordinates of the tile origin
+      const int n = (__ldg(org) + l[0]) + g.L[0] * ((__ldg(org + 1) + l[1]) + g.L[1] * (__ldg(org + 2) + l[2]));
       const double2* hb = x3 < 0 ? c.halo_lo : c.halo_hi;   // NULL at an open face: only the frozen slice asks
       if (hb) {
 #pragma unroll
@@ -598,7 +599,7 @@ __device__ __noinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, c
     } else {
       const double2* src = c.U + field_offset(g, 4 * NCU, p, t, dir * NCU, j);
 #pragma unroll
-      for (int k = 0; k < NCU; k++) v[k] = __ldg(src + (size_t)k * g.TV);
+      for (int k = 0; k < NCU; k++) v[k] = __ldg(src + (size_t)k * CT_TV);
       recon_row3<RECON>(v);
     }
 #pragma unroll
@@ -690,7 +691,7 @@ __global__ void __launch_bounds__(CT_THREADS, 2) clover_tile_kernel(const Clover
   typedef typename vec2<T>::type T2;
   T2* out0 = A + field_offset(g, 36, p, tile, 0, j);
   const double2* own = c.U + field_offset(g, RECON == 12 ? 24 : 36, p, tile, 0, j);
-  const size_t TV = g.TV;
+  constexpr size_t TV = CT_TV;
   auto put = [&](int ch, int idx, double x, double y) {
     if (wr) {
       T2 v;

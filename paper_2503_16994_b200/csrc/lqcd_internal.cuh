@@ -33,7 +33,7 @@ struct Geom {
   int edges;      // LQCD_BC_SLAB: LQCD_SLAB_OPEN_LO | LQCD_SLAB_OPEN_HI (faces that are open boundaries of the lattice)
   long long Vh;   // sites of one parity
   // device table, TILE_TAB ints per tile: linear index of the 8 neighbour tiles (2*mu + (0: +mu, 1: -mu)),
-  // then the time coordinate of the tile origin (library-owned, built by lqcd_geom_create)
+  // then the time coordinate of the tile origin and its three space coordinates (library-owned, built by lqcd_geom_create)
   const int* tile_tab;
   unsigned int* sched;   // SCHED_SLOTS pairs of counters for the pipeline kernel's tile scheduler (library-owned, zeroed)
   int sm_count;     // host-side launch configuration (SMs, opt-in shared memory per CTA)
