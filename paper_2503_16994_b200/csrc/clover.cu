@@ -490,7 +490,7 @@ __device__ __forceinline__ void recon_row3(double2 (&v)[9]) {
 // own: the thread's own links, element offset of row 0 of U_0(x) in the gauge field; ra / rb: where they go
 template <int RECON>
 __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, const int* sNb, const uint32_t* tb, int mu, int nu,
-                                            const double2* own, int ra, int rb) {
+                                            const double2* own, int ra, int rb, m3& Umu) {
   const Geom& g = c.g;
   constexpr int NCU = RECON == 12 ? 6 : 9;
   double2 va[9], vb[9];
@@ -523,6 +523,8 @@ __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, con
 #pragma unroll
   for (int k = 0; k < 9; k++) sU[k * CT_NR + ra] = va[k];
 #pragma unroll
+  for (int k = 0; k < 9; k++) Umu.e[k / 3][k % 3] = va[k];   // stays in registers: first and last link of the leaf chain
+#pragma unroll
   for (int k = 0; k < 9; k++) sU[k * CT_NR + rb] = vb[k];
 #pragma unroll
   for (int it = 0; it < CT_REG; it++) {
@@ -552,7 +554,7 @@ __device__ __forceinline__ void stage_plane(const CloverCtx& c, double2* sU, con
 // field W' (D7); LQCD_BC_SLAB, slices outside the slab come from the gauge halos.  One link at a time.
 template <int RECON>
 __device__ __forceinline__ void stage_plane_edge(const CloverCtx& c, double2* sU, const int* sNb, const uint32_t* tb, int mu, int nu, int t0,
-                                              const double2* own, int ra, int rb) {
+                                              const double2* own, int ra, int rb, m3& Umu) {
   const Geom& g = c.g;
   constexpr int NCU = RECON == 12 ? 6 : 9;
 #pragma unroll 1
@@ -563,6 +565,10 @@ __device__ __forceinline__ void stage_plane_edge(const CloverCtx& c, double2* sU
     recon_row3<RECON>(v);
 #pragma unroll
     for (int k = 0; k < 9; k++) sU[k * CT_NR + (w ? rb : ra)] = v[k];
+    if (w == 0) {
+#pragma unroll
+      for (int k = 0; k < 9; k++) Umu.e[k / 3][k % 3] = v[k];
+    }
   }
   const bool sf = (g.bc == LQCD_BC_SF_ORBI || g.bc == LQCD_BC_SF_AFWB) || (g.bc == LQCD_BC_SLAB && (g.edges & LQCD_SLAB_SF_HI));
 #pragma unroll 1
@@ -615,12 +621,12 @@ __device__ __forceinline__ m3 lds_link(const double2* sU, int r) {
 }
 
 // i F^_{mu nu} of the thread's site from the staged boxes: ra / rb = the site's index in the U_mu / U_nu box,
-// (am, an) / (bm, bn) = the strides of a step along mu / nu in them.  Consecutive leaves share a link.
-__device__ __forceinline__ void i_fhat_staged(const double2* sU, int ra, int am, int an, int rb, int bm, int bn, double (&h)[9]) {
+// (am, an) / (bm, bn) = the strides of a step along mu / nu in them.  Consecutive leaves share a link: 11 reads.
+__device__ __forceinline__ void i_fhat_staged(const double2* sU, const m3& Umu, int ra, int am, int an, int rb, int bm, int bn,
+                                              double (&h)[9]) {
   m3 Q, t, t2, W, H;
-  H = lds_link(sU, ra);                      // U_mu(x)
   W = lds_link(sU, rb + bm);                 // U_nu(x+mu)
-  mul_op<false, false, false>(t, H, W);
+  mul_op<false, false, false>(t, Umu, W);       // U_mu(x) (the thread's own link, kept in registers by the staging)
   W = lds_link(sU, ra + an);                 // U_mu(x+nu)^+
   mul_op<false, true, false>(t2, t, W);
   H = lds_link(sU, rb);                      // U_nu(x)^+ ... and first of leaf 2
@@ -641,8 +647,7 @@ __device__ __forceinline__ void i_fhat_staged(const double2* sU, int ra, int am,
   mul_op<true, false, false>(t, H, W);
   W = lds_link(sU, rb + bm - bn);            // U_nu(x+mu-nu)
   mul_op<false, false, false>(t2, t, W);
-  W = lds_link(sU, ra);                      // U_mu(x)^+
-  mul_op<false, true, true>(Q, t2, W);
+  mul_op<false, true, true>(Q, t2, Umu);        // U_mu(x)^+
 #pragma unroll
   for (int i = 0; i < 3; i++) h[i] = -0.25 * Q.e[i][i].y;
   h[3] = -(Q.e[1][0].y + Q.e[0][1].y) * 0.125;  h[4] = (Q.e[1][0].x - Q.e[0][1].x) * 0.125;
@@ -717,14 +722,15 @@ __global__ void __launch_bounds__(CT_THREADS, 2) clover_tile_kernel(const Clover
         if (d == mu) { am = ba.S[d]; bm = bb.S[d]; }
         if (d == nu) { an = ba.S[d]; bn = bb.S[d]; }
       }
+      m3 Umu;
       __syncthreads();   // the previous plane has been read by every thread
-      if (edge && nu == 3) stage_plane_edge<RECON>(c, sU, sNb, tb, mu, nu, t0, own, ra, rb);
-      else stage_plane<RECON>(c, sU, sNb, tb, mu, nu, own, ra, rb);
+      if (edge && nu == 3) stage_plane_edge<RECON>(c, sU, sNb, tb, mu, nu, t0, own, ra, rb, Umu);
+      else stage_plane<RECON>(c, sU, sNb, tb, mu, nu, own, ra, rb, Umu);
       __syncthreads();
       if (half == 0) {
-        i_fhat_staged(sU, ra, am, an, rb, bm, bn, e);
+        i_fhat_staged(sU, Umu, ra, am, an, rb, bm, bn, e);
       } else {
-        i_fhat_staged(sU, ra, am, an, rb, bm, bn, h);
+        i_fhat_staged(sU, Umu, ra, am, an, rb, bm, bn, h);
       }
     }
     // e = i E_k, h = i B_k;  G_k = kappa csw i(+-E_k - B_k) for the two chiral blocks
