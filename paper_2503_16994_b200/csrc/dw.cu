@@ -113,6 +113,10 @@ __device__ __forceinline__ void hop_dir(const T2<T>* __restrict__ psi, const T2<
   }
 }
 
+#ifndef PIPE_NSPB32
+#define PIPE_NSPB32 2
+#endif
+
 // ---- packed Hermitian 6x6 block times 6-vector, both chiralities (D5) ------------------------------
 // per chirality 18 complex slots: (d0,d1) (d2,d3) (d4,d5), then the strict lower triangle row by row.
 template <typename T>
@@ -371,10 +375,14 @@ struct CloverStage<T, C0, 0> {
 // With both fixed at compile time every shared-memory access of the arithmetic warps is an immediate offset from
 // one base register, and the two halo buffers interleave into rows of 2*PIPE_NF = PIPE_TV columns, i.e. halo rows
 // have the same stride as tile rows and a hop needs no stride select.
+// Spinor-tile buffers of the pipeline kernels.  With one buffer the next tile's spinor can only be requested once the
+// arithmetic warps are done with the hops of this one, and its trip from DRAM is covered by the clover stages alone;
+// fp32 has the shared memory for a second buffer (fp64 does not), and the request then goes out a whole tile ahead.
+template <typename T> __host__ __device__ constexpr int pipe_nspb() { return sizeof(T) == 4 ? PIPE_NSPB32 : 1; }
 enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12, PIPE_TV = 128, PIPE_NF = 64,
        PIPE_TQ = 4 };
 struct PipeBars {
-  uint64_t full_sp, empty_sp;
+  uint64_t full_sp[2], empty_sp[2];   // spinor tile buffer(s): one in fp64, two in fp32 (pipe_nspb)
   uint64_t full_h[4], empty_h[4];   // two halo buffers (full lattice), three (half lattice)
   uint64_t full[PIPE_MAX_SLOTS], empty[PIPE_MAX_SLOTS];
   uint64_t tq_full[PIPE_TQ], tq_empty[PIPE_TQ];   // tile queue: the producer lane tells the other warps which tile is next
@@ -550,13 +558,16 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   const int tid = threadIdx.x;
   const int lane = tid & 31;
   const int warp = tid >> 5;
-  T2<T>* sp = reinterpret_cast<T2<T>*>(smem_raw);   // [2][12][TV] spinor tile
-  T2<T>* ring = sp + 24 * TV;                       // nslot x [2][NCU][TV]
+  constexpr int NSPB = pipe_nspb<T>();
+  T2<T>* sp0 = reinterpret_cast<T2<T>*>(smem_raw);  // NSPB x [2][12][TV] spinor tile
+  T2<T>* ring = sp0 + NSPB * 24 * TV;               // nslot x [2][NCU][TV]
   T2<T>* halo = ring + nslot * 2 * NCU * TV;        // [24 + NCU][PIPE_TV]: both halo buffers
   PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * TV);
   if (tid == 0) {
-    mbar_init(&bars->full_sp, 1);
-    mbar_init(&bars->empty_sp, PIPE_CONS_WARPS);
+    for (int i = 0; i < NSPB; i++) {
+      mbar_init(&bars->full_sp[i], 1);
+      mbar_init(&bars->empty_sp[i], PIPE_CONS_WARPS);
+    }
     for (int i = 0; i < nhb; i++) {
       mbar_init(&bars->full_h[i], PIPE_HALO_THREADS);
       mbar_init(&bars->empty_h[i], PIPE_CONS_WARPS);
@@ -603,11 +614,22 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         const int tile = unit / nsplit;
         for (int rhs = r0; rhs < r0 + nper; rhs++, k++) {   // the unit's right-hand sides back to back: links and clover
                                                        // blocks of the 2nd..nth pass come out of L2
-          if (k == 0) {
-            mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
+          // spinor of pass kk (buffer kk % NSPB): its previous occupant, pass kk - NSPB, must have been released
+          auto request_spinor = [&](const int kk, const int t, const int r) {
+            const int b = kk % NSPB;
+            if (kk >= NSPB) mbar_wait_relaxed(&bars->empty_sp[b], (uint32_t)((kk / NSPB - 1) & 1));
+            mbar_arrive_expect_tx(&bars->full_sp[b], 2 * sp_bytes);
             for (int p = 0; p < 2; p++)
-              bulk_g2s(sp + (p * 12) * TV, a.in + rhs * a.rhs_stride + field_offset(g, 12, p, tile, 0, 0), sp_bytes, &bars->full_sp);
+              bulk_g2s(sp0 + (b * 24 + p * 12) * TV, a.in + r * a.rhs_stride + field_offset(g, 12, p, t, 0, 0), sp_bytes,
+                       &bars->full_sp[b]);
+          };
+          int next = tile, nr = rhs + 1;
+          if (nr == r0 + nper) {
+            next = tile_after >= 0 ? tile_after / nsplit : -1;
+            nr = tile_after >= 0 ? (tile_after % nsplit) * nper : 0;
           }
+          if (k == 0) request_spinor(0, tile, rhs);
+          if (NSPB > 1 && next >= 0) request_spinor(k + 1, next, nr);   // a whole pass ahead
 #pragma unroll 1
           for (int st = 0; st < 4 + NSTC; st++) {   // stage order: L0 L1 [A+] L2 L3 [A-]  (consumer loop below)
             constexpr int H = NSTC / 2;
@@ -632,18 +654,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             }
             rp.advance(nslot);
           }
-          int next = tile, nr = rhs + 1;
-          if (nr == r0 + nper) {
-            next = tile_after >= 0 ? tile_after / nsplit : -1;
-            nr = tile_after >= 0 ? (tile_after % nsplit) * nper : 0;
-          }
-          if (next >= 0) {  // spinor of the next pass: its buffer is released after this pass's hops
-            mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
-            mbar_arrive_expect_tx(&bars->full_sp, 2 * sp_bytes);
-            for (int p = 0; p < 2; p++)
-              bulk_g2s(sp + (p * 12) * TV, a.in + nr * a.rhs_stride + field_offset(g, 12, p, next, 0, 0), sp_bytes,
-                       &bars->full_sp);
-          }
+          // one buffer: the spinor of the next pass is requested when this pass's hops have released the buffer
+          if (NSPB == 1 && next >= 0) request_spinor(k + 1, next, nr);
         }
         }
         tile = tile_after;
@@ -696,7 +708,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       cx<T> acc[12], v[12], res[12];
 #pragma unroll
       for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
-      mbar_wait(&bars->full_sp, (uint32_t)(k & 1));
+      const T2<T>* sp = sp0 + (k % NSPB) * 24 * TV;
+      mbar_wait(&bars->full_sp[k % NSPB], (uint32_t)((k / NSPB) & 1));
 #define LQCD_HOP_STAGE(MU)                                                                                       \
       {                                                                                                          \
         const int b = hp.slot;                                                                                   \
@@ -756,7 +769,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       // stage costs 1.2 % at 48^3 x 96.)
       release_fence();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&bars->empty_sp);   // spinor tile no longer needed: next tile's may land
+      if (lane == 0) mbar_arrive(&bars->empty_sp[k % NSPB]);   // spinor tile no longer needed: the next but NSPB-1 may land
       if (DIAG == DIAG_PRE) {
         CloverPipe<T, NCU, NSTC / 2, NSTC>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
         if (live) {
@@ -906,14 +919,18 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   const int lane = tid & 31;
   const int warp = tid >> 5;
   const int p = a.parity, q = 1 - p;
-  T2<T>* sp_in = reinterpret_cast<T2<T>*>(smem_raw);        // [12][TV] input spinor, parity q; exchange area after the hops
-  T2<T>* sp_self = sp_in + 12 * TV;                         // [12][TV] self spinor, parity p (SELF)
-  T2<T>* ring = sp_self + (SELF ? 12 * TV : 0);             // nslot x [2][NCU][TV] (block stages use the first 9 rows)
+  constexpr int NSPB = pipe_nspb<T>();                      // spinor buffers (fp32: two)
+  constexpr int SPW = SELF ? 24 : 12;                       // rows of one spinor buffer:
+  T2<T>* sp_base = reinterpret_cast<T2<T>*>(smem_raw);      //   [12][TV] input spinor, parity q; exchange area after the hops
+                                                            //   [12][TV] self spinor, parity p (SELF)
+  T2<T>* ring = sp_base + NSPB * SPW * TV;                  // nslot x [2][NCU][TV] (block stages use the first 9 rows)
   T2<T>* halo = ring + nslot * 2 * NCU * TV;                // [24 + NCU][HALF_HS]: three halo buffers of 32 columns
   PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * HALF_HS);
   if (tid == 0) {
-    mbar_init(&bars->full_sp, 1);
-    mbar_init(&bars->empty_sp, PIPE_CONS_WARPS);
+    for (int i = 0; i < NSPB; i++) {
+      mbar_init(&bars->full_sp[i], 1);
+      mbar_init(&bars->empty_sp[i], PIPE_CONS_WARPS);
+    }
     for (int i = 0; i < HALF_NHB; i++) {
       mbar_init(&bars->full_h[i], PIPE_HALO_THREADS);
       mbar_init(&bars->empty_h[i], PIPE_CONS_WARPS);
@@ -945,15 +962,21 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         int tile = blockIdx.x;
         int tile_after = next_tile(NUNITS, a.sched, tile);
         tq_push(bars, kt++, tile);
-        auto load_spinors = [&](const int t) {
-          mbar_arrive_expect_tx(&bars->full_sp, (SELF ? 2 : 1) * sp_bytes);
-          bulk_g2s(sp_in, a.in + field_offset(g, 12, q, t, 0, 0), sp_bytes, &bars->full_sp);
-          if (SELF) bulk_g2s(sp_self, a.self + field_offset(g, 12, p, t, 0, 0), sp_bytes, &bars->full_sp);
+        // spinors of the kk-th tile of this CTA (buffer kk % NSPB): the buffer's previous occupant, tile kk - NSPB, must
+        // have been released (after its exchange)
+        auto load_spinors = [&](const int kk, const int t) {
+          const int b = kk % NSPB;
+          if (kk >= NSPB) mbar_wait_relaxed(&bars->empty_sp[b], (uint32_t)((kk / NSPB - 1) & 1));
+          T2<T>* sp_in = sp_base + b * SPW * TV;
+          mbar_arrive_expect_tx(&bars->full_sp[b], (SELF ? 2 : 1) * sp_bytes);
+          bulk_g2s(sp_in, a.in + field_offset(g, 12, q, t, 0, 0), sp_bytes, &bars->full_sp[b]);
+          if (SELF) bulk_g2s(sp_in + 12 * TV, a.self + field_offset(g, 12, p, t, 0, 0), sp_bytes, &bars->full_sp[b]);
         };
-        load_spinors(tile);
+        load_spinors(0, tile);
         while (tile >= 0) {
           tq_push(bars, kt++, tile_after);
           const int tile_after2 = tile_after >= 0 ? next_tile(NUNITS, a.sched, tile_after) : -1;
+          if (NSPB > 1 && tile_after >= 0) load_spinors(k + 1, tile_after);   // a whole tile ahead
 #pragma unroll 1
           for (int st = 0; st < 4 + NSTC; st++) {   // L0 L1 L2 L3 C0 C1 C2 C3
             mbar_wait_relaxed(&bars->empty[rp.slot], rp.ph ^ 1u);
@@ -968,10 +991,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
             }
             rp.advance(nslot);
           }
-          if (tile_after >= 0) {   // spinors of the next tile: the buffers are released after this tile's exchange
-            mbar_wait_relaxed(&bars->empty_sp, (uint32_t)(k & 1));
-            load_spinors(tile_after);
-          }
+          if (NSPB == 1 && tile_after >= 0) load_spinors(k + 1, tile_after);   // one buffer: once this tile has released it
           k++;
           tile = tile_after;
           tile_after = tile_after2;
@@ -1018,7 +1038,9 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       cx<T> acc[12];
 #pragma unroll
       for (int c = 0; c < 12; c++) acc[c] = cx<T>(0, 0);
-      mbar_wait(&bars->full_sp, (uint32_t)(k & 1));
+      T2<T>* sp_in = sp_base + (k % NSPB) * SPW * TV;
+      const T2<T>* sp_self = sp_in + 12 * TV;
+      mbar_wait(&bars->full_sp[k % NSPB], (uint32_t)((k / NSPB) & 1));
 #define LQCD_HALF_HOP(MU)                                                                                              \
       {                                                                                                                \
         const int b = hp.slot;                                                                                         \
@@ -1081,7 +1103,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       }
       release_fence();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&bars->empty_sp);   // both spinor buffers may be overwritten
+      if (lane == 0) mbar_arrive(&bars->empty_sp[k % NSPB]);   // both spinor buffers may be overwritten
       if (NSTC > 0) {
         // DIAG_PRE: m = hops - (1/k) A self, result = -k m;  DIAG_POST: result = B (hops)
         if (DIAG == DIAG_POST) {
@@ -1219,13 +1241,14 @@ static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
   if (dw_mode() != MODE_PIPE || parity >= 0 || diag == DIAG_POST) return c;
   if (g.b[0] != 4 || g.b[1] != 4 || g.b[2] != 4 || g.b[3] != 4 || g.tile_tab == nullptr) return c;   // PIPE_TV, PIPE_NF
   const int ncu = recon == 12 ? 6 : 9;
-  const size_t sp = (size_t)24 * g.TV * sizeof(T2<T>);
+  const size_t sp = (size_t)pipe_nspb<T>() * 24 * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
   const size_t halo = (size_t)(24 + ncu) * PIPE_TV * sizeof(T2<T>);   // both buffers
   const size_t budget = (size_t)g.smem_optin - 256;   // 256 B: the kernel's static shared memory
   if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
   int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
-  if (nslot > 4) nslot = 4;   // measured: a deeper ring only lets the stream run further ahead of the halos (fp32)
+  if (nslot > 4) nslot = 4;   // measured: a deeper ring only lets the stream run further ahead of the halos (fp32, with two
+                              // spinor buffers: 4 / 6 / 8 slots 1.58 / 1.68 / 1.74 ms at 48^3 x 96)
   const int e = env_int("LQCD_NSLOT", nslot);
   if (e >= 2 && e <= nslot) nslot = e;
   c.use = true;
@@ -1245,13 +1268,15 @@ static PipeCfg pipe_half_config(const Geom& g, int recon, int diag, int parity) 
   if (g.b[0] != 4 || g.b[1] != 4 || g.b[2] != 4 || g.b[3] != 4 || g.tile_tab == nullptr) return c;
   if (env_int("LQCD_EO_PIPE", 1) == 0) return c;   // experiment switch: the one-thread-per-site kernel instead
   const int ncu = recon == 12 ? 6 : 9;
-  const size_t sp = (size_t)(diag == DIAG_POST ? 12 : 24) * g.TV * sizeof(T2<T>);
+  const size_t sp = (size_t)pipe_nspb<T>() * (diag == DIAG_POST ? 12 : 24) * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
   const size_t halo = (size_t)(24 + ncu) * HALF_HS * sizeof(T2<T>);
   const size_t budget = (size_t)g.smem_optin - 256;
   if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
   int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
-  if (nslot > 4) nslot = 4;
+  // ring depth: with two spinor buffers (fp32) the producer is no longer held back by the spinor release and a deeper
+  // ring pays: D^ fp32 at 32^3 x 64 with 4 / 5 / 6 / 7 / 8 slots 0.462 / 0.440 / 0.439 / 0.454 / 0.458 ms
+  { const int cap = pipe_nspb<T>() > 1 ? 6 : 4; if (nslot > cap) nslot = cap; }
   const int e = env_int("LQCD_NSLOT", nslot);
   if (e >= 2 && e <= nslot) nslot = e;
   c.use = true;
