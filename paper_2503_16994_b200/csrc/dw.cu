@@ -335,7 +335,7 @@ __global__ void __launch_bounds__(128, 3) dw_kernel_h(const Geom g, const DwArgs
 //   * warps 9-11: the halo of direction mu -- the spinors on the two faces of the neighbour tiles and the
 //     links U_mu(x - mu) leaving the backward face -- is gathered element by element with per-thread
 //     asynchronous copies (cp.async, SASS LDGSTS; they complete on an mbarrier, occupy no registers) into a
-//     double-buffered halo area; the stage order (below) gives every halo three stages of lead.
+//     double-buffered halo area; the stage order (below) gives every halo two (fp64) or three (fp32) stages of lead.
 //   * warps 0-7: 2*TV consumer threads, one per site (both parities of the tile), run the spin-projected
 //     hops and the clover multiply purely out of shared memory.
 // =====================================================================================================
@@ -379,6 +379,12 @@ struct CloverStage<T, C0, 0> {
 // arithmetic warps are done with the hops of this one, and its trip from DRAM is covered by the clover stages alone;
 // fp32 has the shared memory for a second buffer (fp64 does not), and the request then goes out a whole tile ahead.
 template <typename T> __host__ __device__ constexpr int pipe_nspb() { return sizeof(T) == 4 ? PIPE_NSPB32 : 1; }
+// Clover stages placed between the two pairs of hop stages (the rest follows the last hop).  fp32: half of them, so that
+// every halo has three stages of lead.  fp64, with its single spinor buffer: one -- the spinor tile is released after
+// the last hop, and the more stages follow it the more time the next tile's spinor has to arrive from DRAM; the halos,
+// which mostly come out of L2, make do with two stages of lead (measured: 2.948 -> 2.914 ms at 48^3 x 96; none early:
+// 3.003 ms; fp32 with one early stage: 1.573 -> 1.593 ms).
+template <typename T> __host__ __device__ constexpr int pipe_early_stages(int nstc) { return sizeof(T) == 8 ? (nstc > 0 ? 1 : 0) : nstc / 2; }
 enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX_SLOTS = 12, PIPE_TV = 128, PIPE_NF = 64,
        PIPE_TQ = 4 };
 struct PipeBars {
@@ -631,8 +637,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           if (k == 0) request_spinor(0, tile, rhs);
           if (NSPB > 1 && next >= 0) request_spinor(k + 1, next, nr);   // a whole pass ahead
 #pragma unroll 1
-          for (int st = 0; st < 4 + NSTC; st++) {   // stage order: L0 L1 [A+] L2 L3 [A-]  (consumer loop below)
-            constexpr int H = NSTC / 2;
+          for (int st = 0; st < 4 + NSTC; st++) {   // stage order: L0 L1 [H clover stages] L2 L3 [the rest]  (consumer loop below)
+            constexpr int H = pipe_early_stages<T>(NSTC);
             int mu = -1, cs = -1;
             if (st < 2) mu = st;
             else if (st < 2 + H) cs = st - 2;
@@ -726,8 +732,9 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         rp.advance(nslot);                                                                                       \
         hp.advance(nhb);                                                                                         \
       }
-      // Stage order H0 H1 [A+ stages] H2 H3 [A- stages]: with two halo buffers every halo then has three stages
-      // of lead.  With the clover term ONE accumulator serves both: acc = sum of hops - (1/k) A psi, result = -k acc,
+      // Stage order H0 H1 [early clover stages] H2 H3 [the other clover stages] (pipe_early_stages): clover stages
+      // between the hop pairs give the halos lead, clover stages after the last hop give the next spinor tile lead.
+      // With the clover term ONE accumulator serves both: acc = sum of hops - (1/k) A psi, result = -k acc,
       // so that no second 12-component register set is live during the hops.
       const T2<T>* sv = sp + (p * 12) * TV + j;
       LQCD_HOP_STAGE(0)
@@ -742,7 +749,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           }
           if (a.tm != T(0)) add_twist<T, 0, 6>(a.tm, v, acc);   // acc carries -(1/k) (A + i tm gamma5) psi
         }
-        CloverPipe<T, NCU, 0, NSTC / 2>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
+        CloverPipe<T, NCU, 0, pipe_early_stages<T>(NSTC)>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
       }
       LQCD_HOP_STAGE(2)
       LQCD_HOP_STAGE(3)
@@ -771,7 +778,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->empty_sp[k % NSPB]);   // spinor tile no longer needed: the next but NSPB-1 may land
       if (DIAG == DIAG_PRE) {
-        CloverPipe<T, NCU, NSTC / 2, NSTC>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
+        CloverPipe<T, NCU, pipe_early_stages<T>(NSTC), NSTC>::run(bars, ring, rp, nslot, TV, (p * NCU) * TV + j, live, lane, v, acc);
         if (live) {
 #pragma unroll
           for (int c = 0; c < 12; c++) res[c] = cx<T>(-a.k * acc[c].re, -a.k * acc[c].im);
