@@ -708,8 +708,8 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     if (unit < 0) break;
     const int tile = unit / nsplit, r0 = (unit % nsplit) * nper;
     for (int rhs = r0; rhs < r0 + nper; rhs++, k++) {
-      const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
-      const int x3 = __ldg(tab + 8) + l[3];
+      // the time coordinate matters only where time is not periodic: no load (and no wait for it) on periodic lattices
+      const int x3 = nonper ? __ldg(g.tile_tab + (size_t)tile * TILE_TAB + 8) + l[3] : 0;
       const bool live = !(nonper && frozen_slice(g, x3));
       cx<T> acc[12], v[12], res[12];
 #pragma unroll
@@ -1039,8 +1039,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
     for (int kt = 0;; kt++, k++) {
       const int tile = tq_pop(bars, kt, lane);
       if (tile < 0) break;
-      const int* tab = g.tile_tab + (size_t)tile * TILE_TAB;
-      const int x3 = __ldg(tab + 8) + l[3];
+      const int x3 = nonper ? __ldg(g.tile_tab + (size_t)tile * TILE_TAB + 8) + l[3] : 0;   // (see dw_pipe_kernel)
       const bool live = !(nonper && frozen_slice(g, x3));
       cx<T> acc[12];
 #pragma unroll
