@@ -144,6 +144,32 @@ def test_dw_apply_multi(mode, prec, nrhs, grid):
     lat.close()
 
 
+@pytest.mark.parametrize("nrhs", [1, 7, 64])
+def test_dw_apply_multi_column_counts(nrhs):
+    """The limits of lqcd_dw_apply_multi: one column, a prime number of columns (no split into work units possible), the
+    maximum of 64 (four work units of 16) -- each column bit-identical to a single application -- and 0 / 65 rejected."""
+    L, kappa, csw = (8, 8, 4, 8), 0.137, 1.9
+    dev = torch.device("cuda", torch.cuda.current_device())
+    lat = Lattice(L)
+    lat.set_gauge(synth.smooth_gauge_torch(L, 91, dev))
+    lat.build_clover(kappa, csw)
+    fb = B.field_bytes(lat.g, B.FIELD_SPINOR)
+    src = torch.empty(nrhs * fb, dtype=torch.uint8, device="cuda")
+    dst = torch.full((nrhs * fb,), 0x7F, dtype=torch.uint8, device="cuda")
+    for n in range(nrhs):
+        src[n * fb:(n + 1) * fb].copy_(lat.spinor(synth.gaussian_spinor_torch(L, 92 + n, dev)))
+    B.dw_apply_multi(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, dst, nrhs)
+    single = lat.alloc(B.FIELD_SPINOR)
+    for n in range(nrhs):
+        B.dw_apply(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src[n * fb:(n + 1) * fb], single)
+        torch.cuda.synchronize()
+        assert torch.equal(single, dst[n * fb:(n + 1) * fb]), n
+    for bad in (0, 65):
+        with pytest.raises(B.LqcdError):
+            B.dw_apply_multi(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], src, dst, bad)
+    lat.close()
+
+
 def test_kappa_must_be_positive():
     """kappa <= 0 (or not finite) is refused by every operator / solver entry point instead of producing NaN on the
     pipeline kernel (which folds the diagonal term in as -(1/kappa) A psi) and A psi on the others."""
