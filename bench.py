@@ -625,6 +625,20 @@ def run_config3(torch, B, synth, peak):
             "outer": [i["outer"] for i in infos],
             "max_rel_resid_normal": max(i["rel_resid_normal"] for i in infos),
             "max_rel_resid_true": max(i["rel_resid_true"] for i in infos)}
+    # the same 12 columns solved in lock step (lqcd_propagator_batched: every stencil pass takes all columns)
+    wsb = torch.empty(B.cg_multi_workspace_bytes(g, 12), dtype=torch.uint8, device="cuda")
+    srcs = torch.empty_like(cols)
+    t0 = time.perf_counter()
+    infos = B.propagator_batched(g, kappa, S.U[(B.F64, 18)], S.A[B.F64], y, cols, srcs, wsb, tol=1e-10, maxiter=10000)
+    dt = time.perf_counter() - t0
+    one = out["a8_propagator_24x24x24x48_open_plain_f64"]
+    out["a8_propagator_24x24x24x48_open_plain_f64_batched"] = {
+        "seconds_12_columns": round(dt, 3), "iterations": [i["iters"] for i in infos],
+        "vs_column_by_column": round(dt / one["seconds_12_columns"], 3),
+        "same_iteration_counts": [i["iters"] for i in infos] == one["iterations"],
+        "max_rel_resid_normal": max(i["rel_resid_normal"] for i in infos),
+        "max_rel_resid_true": max(i["rel_resid_true"] for i in infos)}
+    del wsb, srcs
     S.close()
     del S, cols, ws, U32
     torch.cuda.empty_cache()

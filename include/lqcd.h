@@ -148,6 +148,30 @@ lqcd_status lqcd_propagator(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_
 lqcd_status lqcd_spinor_norm2(const lqcd_geom* g, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host, void* stream);
 lqcd_status lqcd_spinor_dot(const lqcd_geom* g, const void* u, const void* v, int half, lqcd_prec prec, void* workspace, double* result_host /* re, im */, void* stream);
 
+/* SURVEY.md 8(f) NEXT-1 carried into the solver (the 12 colour-spin sources of propagator!):
+ * nrhs (1..64) independent systems D x_n = b_n solved by CG on the normal equations IN LOCK STEP -- every stencil
+ * pass is one lqcd_dw_apply_multi over all columns (links and clover blocks are fetched once per tile for all of
+ * them) with the |t|^2 / r -= alpha q / |r|^2 epilogues fused per column; alpha, beta, the iteration count and the
+ * convergence flag are kept per column on the device, and a column that has converged is frozen (alpha = 0) while
+ * the others go on.  Per column the arithmetic is that of lqcd_cg_solve (same iterates, same iteration count).
+ *   b, x      : DEVICE, nrhs internal fp64 spinor fields back to back (lqcd_field_bytes(SPINOR) apart), caller-owned,
+ *               not overlapping; components of b on frozen time slices are ignored (D7)
+ *   workspace : DEVICE, lqcd_cg_multi_workspace_bytes(g, nrhs) bytes (4 nrhs spinor fields + reduction scratch)
+ *   infos     : HOST, nrhs entries; `seconds` is the time of the whole call in every entry
+ * Plain fp64 only: with parm->eo or parm->mixed set, with nrhs == 1, or on a lattice the pipeline kernel does not
+ * serve (tiles other than 4^4), the columns are solved one after the other by lqcd_cg_solve (same results; the fields
+ * those modes need must then be in `f`).  Errors: as lqcd_cg_solve; LQCD_ENOTCONV / LQCD_EBREAKDOWN if any column
+ * failed (lqcd_last_error names the first / the broken one), all infos are filled.
+ * lqcd_propagator_batched: the 12 point-source columns of lqcd_propagator through lqcd_cg_solve_multi; `sources`:
+ * DEVICE scratch for the 12 source fields (12 spinor fields, caller-owned). */
+size_t lqcd_cg_multi_workspace_bytes(const lqcd_geom* g, int nrhs);
+lqcd_status lqcd_cg_solve_multi(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b, void* x,
+                                int nrhs, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* infos, lqcd_recon recon,
+                                void* stream);
+lqcd_status lqcd_propagator_batched(const lqcd_geom* g, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4],
+                                    void* columns, void* sources, void* workspace, const lqcd_cg_parm* parm,
+                                    lqcd_cg_info infos[12], lqcd_recon recon, void* stream);
+
 /* SURVEY.md 8(f) NEXT-2 (PAPER.md:11 "fermionic two point functions", :125 the columns of propagator!): the
  * pseudoscalar two-point function of ncol propagator columns,
  *   C(x4) = sum over x1,x2,x3 of sum over columns, spin, colour of |S(x)|^2      ( = sum_xvec Tr S^+ S ),

@@ -22,7 +22,7 @@ EXPORTS = [
     "lqcd_geom_create", "lqcd_geom_destroy", "lqcd_geom_info", "lqcd_field_bytes",
     "lqcd_gauge_import", "lqcd_gauge_export", "lqcd_spinor_import", "lqcd_spinor_export",
     "lqcd_clover_export", "lqcd_field_to_f32", "lqcd_clover_build", "lqcd_dw_apply", "lqcd_dwdag_apply",
-    "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_propagator", "lqcd_spinor_norm2",
+    "lqcd_dw_eo_apply", "lqcd_point_source", "lqcd_cg_solve", "lqcd_cg_solve_multi", "lqcd_cg_multi_workspace_bytes", "lqcd_propagator_batched", "lqcd_propagator", "lqcd_spinor_norm2",
     "lqcd_spinor_dot", "lqcd_dw_apply_host", "lqcd_host_cache_release", "lqcd_last_error", "lqcd_launch_count", "lqcd_dw_plan",
     "lqcd_set_option", "lqcd_dw_apply_multi", "lqcd_correlator_ps", "lqcd_correlator_ps_static", "lqcd_dw_slab_pack", "lqcd_dw_slab_faces",
     "lqcd_clover_build_slab", "lqcd_cg_solve_slab",
@@ -287,6 +287,41 @@ def propagator(g, kappa, U64, clover64, y, columns, workspace, tol=1e-10, maxite
     yy = (ctypes.c_int * 4)(*[int(v) for v in y])
     st = lib().lqcd_propagator(g, ctypes.byref(d), ctypes.byref(f), yy, _ptr(columns), _ptr(workspace), ctypes.byref(p),
                                infos, recon, _stream(stream))
+    _check(st)
+    return [_info_dict(infos[i], st) for i in range(12)]
+
+
+def cg_multi_workspace_bytes(g, nrhs):
+    lib().lqcd_cg_multi_workspace_bytes.restype = ctypes.c_size_t
+    lib().lqcd_cg_multi_workspace_bytes.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    return int(lib().lqcd_cg_multi_workspace_bytes(g, int(nrhs)))
+
+
+def cg_solve_multi(g, kappa, U64, clover64, b, x, nrhs, workspace, tol=1e-10, maxiter=10000, clover_inv64=None, U32=None,
+                   clover32=None, clover_inv32=None, mixed=False, eo=False, inner_tol=1e-4, check_every=16,
+                   recon=RECON_18, stream=None, raise_on_notconv=True, mu=0.0):
+    """nrhs systems D x_n = b_n in lock step (b, x: nrhs internal fp64 spinor fields back to back); workspace of
+    cg_multi_workspace_bytes(g, nrhs) bytes.  Returns a list of info dicts."""
+    d = _dirac(kappa, mu=mu)
+    f, p = _cg_args(U64, clover64, clover_inv64, U32, clover32, clover_inv32, tol, maxiter, mixed, eo, inner_tol, check_every)
+    infos = (CgInfo * int(nrhs))()
+    st = lib().lqcd_cg_solve_multi(g, ctypes.byref(d), ctypes.byref(f), _ptr(b), _ptr(x), int(nrhs), _ptr(workspace),
+                                   ctypes.byref(p), infos, recon, _stream(stream))
+    if st != OK and not (st == ENOTCONV and not raise_on_notconv):
+        _check(st)
+    return [_info_dict(infos[i], st) for i in range(int(nrhs))]
+
+
+def propagator_batched(g, kappa, U64, clover64, y, columns, sources, workspace, tol=1e-10, maxiter=10000, check_every=16,
+                       recon=RECON_18, stream=None, mu=0.0):
+    """The 12 point-source columns through cg_solve_multi (plain fp64); sources: scratch of 12 spinor fields,
+    workspace: cg_multi_workspace_bytes(g, 12) bytes."""
+    d = _dirac(kappa, mu=mu)
+    f, p = _cg_args(U64, clover64, None, None, None, None, tol, maxiter, False, False, 1e-4, check_every)
+    infos = (CgInfo * 12)()
+    yy = (ctypes.c_int * 4)(*[int(v) for v in y])
+    st = lib().lqcd_propagator_batched(g, ctypes.byref(d), ctypes.byref(f), yy, _ptr(columns), _ptr(sources), _ptr(workspace),
+                                       ctypes.byref(p), infos, recon, _stream(stream))
     _check(st)
     return [_info_dict(infos[i], st) for i in range(12)]
 

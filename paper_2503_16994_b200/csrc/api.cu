@@ -991,6 +991,118 @@ lqcd_status lqcd_propagator(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_
   return LQCD_OK;
 }
 
+
+// ---- several columns in lock step (SURVEY.md 8(f) NEXT-1 carried into the solver) ----------------------------------
+static size_t multi_partial_len(const Geom& g, int nrhs) {
+  size_t per = (size_t)g.ntiles;
+  const size_t np = (size_t)reduce_blocks_max();
+  if (np > per) per = np;
+  return (size_t)nrhs * per + 64;
+}
+size_t lqcd_cg_multi_workspace_bytes(const lqcd_geom* h, int nrhs) {
+  if (!h || nrhs < 1 || nrhs > 64) return 0;
+  const Geom& g = h->g;
+  const size_t sp64 = align256((size_t)2 * g.Vh * 12 * sizeof(double2));
+  size_t multi = (size_t)4 * nrhs * sp64 + align256(multi_partial_len(g, nrhs) * sizeof(double)) + align256(64) +
+                 align256((size_t)nrhs * sizeof(CgState)) + align256(2 * sizeof(int)) + 4096;
+  const size_t single = lqcd_field_bytes(h, LQCD_FIELD_WORKSPACE, LQCD_F64, LQCD_RECON_18);
+  return multi > single ? multi : single;
+}
+
+lqcd_status lqcd_cg_solve_multi(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const void* b, void* x,
+                                int nrhs, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info* infos, lqcd_recon recon,
+                                void* stream) {
+  REQUIRE(h && d && f && b && x && workspace && parm && infos, "lqcd_cg_solve_multi: NULL argument");
+  REQUIRE(good_kappa(d), "lqcd_cg_solve_multi: kappa must be positive and finite (got %g)", d->kappa);
+  REQUIRE(nrhs >= 1 && nrhs <= 64, "lqcd_cg_solve_multi: nrhs must be in 1..64");
+  REQUIRE(valid_recon(recon), "lqcd_cg_solve_multi: bad recon");
+  REQUIRE(f->U64, "lqcd_cg_solve_multi: U64 is required");
+  REQUIRE(parm->tol > 0 && parm->maxiter >= 0, "lqcd_cg_solve_multi: bad tol / maxiter");
+  UNSUPPORTED_ON_SLAB(h, "lqcd_cg_solve_multi");
+  DeviceGuard dg(h);
+  const Geom& g = h->g;
+  const size_t fb = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, LQCD_F64, recon);
+  {
+    const char *ib = (const char*)b, *ob = (const char*)x;
+    REQUIRE(ob + (size_t)nrhs * fb <= ib || ib + (size_t)nrhs * fb <= ob, "lqcd_cg_solve_multi: b and x overlap");
+  }
+  SolveCtx c;
+  c.h = h; c.d = d; c.f = f; c.parm = parm; c.recon = (int)recon; c.s = as_stream(stream);
+  Op<double> M = make_op<double>(c, nullptr);
+  M.eo = false;
+  if (parm->eo || parm->mixed || nrhs == 1 || !M.multi_fused_ok()) {
+    // even-odd / mixed solves, and lattices the pipeline kernel does not serve: one column after the other
+    for (int n = 0; n < nrhs; n++) {
+      lqcd_status st = lqcd_cg_solve(h, d, f, (const char*)b + (size_t)n * fb, (char*)x + (size_t)n * fb, workspace, parm, &infos[n],
+                                     recon, stream);
+      if (st != LQCD_OK) return st;
+    }
+    return LQCD_OK;
+  }
+  auto t0 = std::chrono::steady_clock::now();
+  cudaStream_t s = c.s;
+  const size_t nfull = spinor_complex(g);
+  Workspace ws{(char*)workspace, 0};
+  const size_t arr = (size_t)nrhs * nfull * sizeof(double2);
+  void* r = ws.take(arr);
+  void* p = ws.take(arr);
+  void* t = ws.take(arr);
+  void* bm = ws.take(arr);
+  double* partial = (double*)ws.take(multi_partial_len(g, nrhs) * sizeof(double));
+  double* scratch = (double*)ws.take(64);
+  CgState* states = (CgState*)ws.take((size_t)nrhs * sizeof(CgState));
+  int* flags = (int*)ws.take(2 * sizeof(int));
+  std::vector<CgState> hs(nrhs);
+  memset(infos, 0, (size_t)nrhs * sizeof(*infos));
+  if (g.bc != LQCD_BC_PERIODIC) {   // D7: components of b on frozen slices are ignored (as in lqcd_cg_solve)
+    CKS(cudaMemcpyAsync(bm, b, arr, cudaMemcpyDeviceToDevice, s), "copy b");
+    for (int n = 0; n < nrhs; n++) CKS(mask_frozen<double>(g, (double2*)bm + (size_t)n * nfull, s), "mask");
+    b = bm;
+  }
+  CKS(M.apply_multi(b, t, nrhs, true, s), "D^+ b");   // b' in t: copied into r and p before t is first written
+  const int check = parm->check_every > 0 ? parm->check_every : 16;
+  CKS(cg_normal_multi<double>(M, nrhs, t, x, r, p, t, partial, states, flags, parm->tol, parm->maxiter, check, hs.data(), s),
+      "cg_normal_multi");
+  // true residuals with fresh operator applications (R11)
+  CKS(M.apply_multi(x, t, nrhs, false, s), "D x");
+  for (int n = 0; n < nrhs; n++)
+    CKS(xmy<double>((const double2*)b + (size_t)n * nfull, (double2*)t + (size_t)n * nfull, (double2*)t + (size_t)n * nfull, nfull, s), "b - Dx");
+  CKS(M.apply_multi(t, p, nrhs, true, s), "D^+ (b - Dx)");
+  lqcd_status st = LQCD_OK;
+  for (int n = 0; n < nrhs; n++) {
+    double nb = 0, nr = 0, nq = 0;
+    CKS(device_norm2<double>((const double2*)b + (size_t)n * nfull, nfull, partial, scratch, &nb, s), "norm2");
+    CKS(device_norm2<double>((const double2*)t + (size_t)n * nfull, nfull, partial, scratch, &nr, s), "norm2");
+    CKS(device_norm2<double>((const double2*)p + (size_t)n * nfull, nfull, partial, scratch, &nq, s), "norm2");
+    infos[n].iters = hs[n].iters;
+    infos[n].rel_resid_true = nb > 0 ? sqrt(nr / nb) : 0.0;
+    infos[n].rel_resid_normal = hs[n].rho0 > 0 ? sqrt(nq / hs[n].rho0) : 0.0;
+    if (hs[n].breakdown) {
+      set_error("lqcd_cg_solve_multi: column %d: breakdown (NaN or <p,M^+M p> <= 0) at iteration %d", n, hs[n].iters);
+      st = LQCD_EBREAKDOWN;
+    } else if (!hs[n].done && st == LQCD_OK) {
+      set_error("lqcd_cg_solve_multi: column %d not converged after %d iterations", n, hs[n].iters);
+      st = LQCD_ENOTCONV;
+    }
+  }
+  const double secs = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  for (int n = 0; n < nrhs; n++) infos[n].seconds = secs;
+  return st;
+}
+
+lqcd_status lqcd_propagator_batched(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg_fields* f, const int y[4], void* columns,
+                                    void* sources, void* workspace, const lqcd_cg_parm* parm, lqcd_cg_info infos[12],
+                                    lqcd_recon recon, void* stream) {
+  REQUIRE(h && d && f && y && columns && sources && workspace && parm && infos, "lqcd_propagator_batched: NULL argument");
+  DeviceGuard dg(h);
+  const size_t sbytes = lqcd_field_bytes(h, LQCD_FIELD_SPINOR, LQCD_F64, recon);
+  for (int col = 0; col < 12; col++) {
+    lqcd_status st = lqcd_point_source(h, y, col / 3, col % 3, (char*)sources + (size_t)col * sbytes, LQCD_F64, stream);
+    if (st != LQCD_OK) return st;
+  }
+  return lqcd_cg_solve_multi(h, d, f, sources, columns, 12, workspace, parm, infos, recon, stream);
+}
+
 }  // extern "C"
 // ---- host-buffer path -----------------------------------------------------------------------------------------
 // Device scratch, streams and the geometry of the last lqcd_dw_apply_host call are kept (one context per process,

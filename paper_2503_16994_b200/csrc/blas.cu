@@ -115,6 +115,85 @@ __global__ void cg_beta_kernel(CgState* st, const double* partial, int n) {
   }
 }
 
+// ---- the same bookkeeping for nrhs solves in lock step (cg_normal_multi): CTA c serves column c -----------------
+// flags[0]: all columns finished (the stencil launches then return at once), flags[1]: ticket counter of the alpha kernel
+__global__ void cg_init_multi_kernel(CgState* st, const double* partial, int n, double tol, int* flags) {
+  __shared__ double s_red[32];
+  st += blockIdx.x;
+  double s = ordered_sum(partial + (size_t)blockIdx.x * n, n, s_red);
+  if (threadIdx.x == 0) {
+    st->rho = s; st->rho0 = s; st->alpha = 0; st->beta = 0; st->tt = 0; st->rho_new = s;
+    st->tol2 = tol * tol;
+    st->iters = 0; st->breakdown = 0;
+    st->done = (s == 0.0) ? 1 : 0;
+    if (!(s == s)) { st->done = 1; st->breakdown = 1; }
+    if (blockIdx.x == 0) { flags[0] = 0; flags[1] = 0; }
+  }
+}
+// A finished column keeps taking part in the stencil passes (they are per tile, not per column) with alpha = 0, which
+// leaves its r alone; its x and p are no longer touched.  The last CTA to arrive sets the all-finished flag.
+__global__ void cg_alpha_multi_kernel(CgState* st0, const double* partial, int n, int* flags) {
+  __shared__ double s_red[32];
+  CgState* st = st0 + blockIdx.x;
+  if (st->done == 2) { if (threadIdx.x == 0) st->done = 1; }
+  __syncthreads();
+  if (st->done) {
+    if (threadIdx.x == 0) st->alpha = 0;
+  } else {
+    double s = ordered_sum(partial + (size_t)blockIdx.x * n, n, s_red);
+    if (threadIdx.x == 0) {
+      st->tt = s;
+      if (!(s > 0.0)) { st->breakdown = 1; st->done = 1; st->alpha = 0; }
+      else st->alpha = st->rho / s;
+    }
+  }
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(flags + 1, 1) == (int)gridDim.x - 1) {
+      __threadfence();
+      int all = 1;
+      for (unsigned c = 0; c < gridDim.x; c++) all &= (((volatile CgState*)st0)[c].done == 1);
+      flags[0] = all;
+      flags[1] = 0;
+    }
+  }
+}
+__global__ void cg_beta_multi_kernel(CgState* st, const double* partial, int n) {
+  __shared__ double s_red[32];
+  st += blockIdx.x;
+  if (st->done) return;
+  double s = ordered_sum(partial + (size_t)blockIdx.x * n, n, s_red);
+  if (threadIdx.x == 0) {
+    st->rho_new = s;
+    st->iters += 1;
+    if (!(s == s)) { st->breakdown = 1; st->done = 2; st->alpha = 0; }
+    else if (s <= st->tol2 * st->rho0) st->done = 2;  // x += alpha p still pending
+    st->beta = s / st->rho;
+    st->rho = s;
+  }
+}
+// blockIdx.y: column; x, p, r: arrays of fields `stride` complex numbers apart
+template <typename T>
+__global__ void cg_update_xp_multi_kernel(const CgState* st, T2<T>* x, T2<T>* p, const T2<T>* __restrict__ r, size_t n, size_t stride) {
+  st += blockIdx.y;
+  const int done = st->done;
+  if (done == 1) return;
+  x += blockIdx.y * stride; p += blockIdx.y * stride; r += blockIdx.y * stride;
+  const T al = (T)st->alpha, be = (T)st->beta;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    T2<T> xv = x[i], pv = p[i];
+    xv.x = fma(al, pv.x, xv.x);
+    xv.y = fma(al, pv.y, xv.y);
+    x[i] = xv;
+    if (done == 0) {
+      T2<T> rv = r[i];
+      pv.x = fma(be, pv.x, rv.x);
+      pv.y = fma(be, pv.y, rv.y);
+      p[i] = pv;
+    }
+  }
+}
+
 template <typename T>
 __global__ void cg_update_xp_kernel(const CgState* st, T2<T>* x, T2<T>* p, const T2<T>* __restrict__ r, size_t n) {
   const int done = st->done;
@@ -237,6 +316,29 @@ template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void*
   count_launch();
   return cudaGetLastError();
 }
+cudaError_t cg_init_state_multi(CgState* st, int nrhs, const double* partial, int n, double tol, int* flags, cudaStream_t s) {
+  cg_init_multi_kernel<<<nrhs, 1024, 0, s>>>(st, partial, n, tol, flags);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t cg_reduce_alpha_multi(CgState* st, int nrhs, const double* partial, int n, int* flags, cudaStream_t s) {
+  cg_alpha_multi_kernel<<<nrhs, 1024, 0, s>>>(st, partial, n, flags);
+  count_launch();
+  return cudaGetLastError();
+}
+cudaError_t cg_reduce_beta_multi(CgState* st, int nrhs, const double* partial, int n, cudaStream_t s) {
+  cg_beta_multi_kernel<<<nrhs, 1024, 0, s>>>(st, partial, n);
+  count_launch();
+  return cudaGetLastError();
+}
+template <typename T>
+cudaError_t cg_update_xp_multi(const CgState* st, int nrhs, void* x, void* p, const void* r, size_t n, size_t stride, cudaStream_t s) {
+  unsigned bx = (unsigned)ew_blocks(n);
+  if (nrhs > 1 && bx > 2048) bx = 2048;   // nrhs columns share the machine
+  cg_update_xp_multi_kernel<T><<<dim3(bx, (unsigned)nrhs), 256, 0, s>>>(st, (T2<T>*)x, (T2<T>*)p, (const T2<T>*)r, n, stride);
+  count_launch();
+  return cudaGetLastError();
+}
 template <typename T> cudaError_t cg_raxpy_norm(const CgState* st, const void* q, void* r, size_t n, double* partial, cudaStream_t s) {
   cg_raxpy_norm_kernel<T><<<reduce_blocks(n), RB_THREADS, 0, s>>>(st, (const T2<T>*)q, (T2<T>*)r, n, partial);
   count_launch();
@@ -268,6 +370,7 @@ template <typename T> cudaError_t mask_frozen(const Geom& g, void* psi, cudaStre
   template cudaError_t norm2_partial<T>(const void*, size_t, double*, cudaStream_t);                \
   template cudaError_t dot_partial<T>(const void*, const void*, size_t, double*, cudaStream_t);     \
   template cudaError_t cg_update_xp<T>(const CgState*, void*, void*, const void*, size_t, cudaStream_t); \
+  template cudaError_t cg_update_xp_multi<T>(const CgState*, int, void*, void*, const void*, size_t, size_t, cudaStream_t); \
   template cudaError_t axpy<T>(double, const void*, void*, size_t, cudaStream_t);                   \
   template cudaError_t cg_raxpy_norm<T>(const CgState*, const void*, void*, size_t, double*, cudaStream_t); \
   template cudaError_t xmy<T>(const void*, const void*, void*, size_t, cudaStream_t);               \

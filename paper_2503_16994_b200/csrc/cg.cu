@@ -81,6 +81,38 @@ cudaError_t Op<T>::apply_multi(const void* in, void* out, int nrhs, bool dagger,
   return launch_dw<T>(geom->g, a, recon, A ? DIAG_PRE : DIAG_ONE, s);
 }
 
+template <typename T>
+bool Op<T>::multi_fused_ok() const {
+  return !eo && dw_uses_pipe<T>(geom->g, recon, A ? DIAG_PRE : DIAG_ONE, -1);
+}
+
+template <typename T>
+cudaError_t Op<T>::apply_multi_epi(const void* in, void* out, int nrhs, bool dagger, int epi, void* r, const double* alpha,
+                                   int alpha_stride, double* partial, const int* skip, cudaStream_t s) const {
+  DwArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.U = (const T2<T>*)U;
+  a.A = (const T2<T>*)A;
+  a.in = (const T2<T>*)in;
+  a.self = (const T2<T>*)in;
+  a.out = (T2<T>*)out;
+  a.r = (T2<T>*)r;
+  a.alpha = alpha;
+  a.alpha_stride = alpha_stride;
+  a.partial = partial;
+  a.skip = skip;
+  a.k = (T)kappa;
+  a.tm = (T)(2.0 * kappa * (dagger ? -mu : mu));
+  a.has_theta = geom->has_theta;
+  for (int d = 0; d < 4; d++) a.theta[d] = cx<T>((T)geom->th_re[d], (T)geom->th_im[d]);
+  a.dagger = dagger ? 1 : 0;
+  a.parity = -1;
+  a.epi = epi;
+  a.nrhs = nrhs;
+  a.rhs_stride = (long long)2 * geom->g.Vh * 12;
+  return launch_dw<T>(geom->g, a, recon, A ? DIAG_PRE : DIAG_ONE, s);
+}
+
 // out(parity) = self - k * H in   (no clover), used by the even-odd source preparation / reconstruction
 template <typename T>
 cudaError_t Op<T>::hop_xpay(const void* in, const void* self, void* out, double k, int parity, cudaStream_t s) const {
@@ -131,6 +163,42 @@ cudaError_t cg_normal(const Op<T>& M, const void* bprime, void* x, const CgVecto
 }
 
 template <typename T>
+cudaError_t cg_normal_multi(const Op<T>& M, int nrhs, const void* bprime, void* x, void* r, void* p, void* t, double* partial,
+                            CgState* states, int* flags, double tol, int maxiter, int check_every, CgState* host_states,
+                            cudaStream_t s) {
+  const size_t n = M.ncomplex();
+  const size_t bytes = (size_t)nrhs * n * sizeof(T2<T>);
+  const int nt = M.geom->g.ntiles;
+  const int np = reduce_blocks(n);
+  CK(cudaMemsetAsync(x, 0, bytes, s));
+  CK(cudaMemcpyAsync(r, bprime, bytes, cudaMemcpyDeviceToDevice, s));
+  CK(cudaMemcpyAsync(p, bprime, bytes, cudaMemcpyDeviceToDevice, s));
+  for (int c = 0; c < nrhs; c++) CK(norm2_partial<T>((const T2<T>*)r + (size_t)c * n, n, partial + (size_t)c * np, s));
+  CK(cg_init_state_multi(states, nrhs, partial, np, tol, flags, s));
+  if (check_every < 1) check_every = 1;
+  const int astride = (int)(sizeof(CgState) / sizeof(double));
+  int launched = 0;
+  for (;;) {
+    CK(cudaMemcpyAsync(host_states, states, (size_t)nrhs * sizeof(CgState), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    bool all = true;
+    for (int c = 0; c < nrhs; c++) all = all && host_states[c].done != 0;
+    if (all || launched >= maxiter) break;
+    int batch = check_every;
+    if (launched + batch > maxiter) batch = maxiter - launched;
+    for (int it = 0; it < batch; it++) {
+      CK(M.apply_multi_epi(p, t, nrhs, false, EPI_STORE_NORM, nullptr, nullptr, 0, partial, flags, s));
+      CK(cg_reduce_alpha_multi(states, nrhs, partial, nt, flags, s));
+      CK(M.apply_multi_epi(t, nullptr, nrhs, true, EPI_AXPY_NORM, r, &states->alpha, astride, partial, flags, s));
+      CK(cg_reduce_beta_multi(states, nrhs, partial, nt, s));
+      CK(cg_update_xp_multi<T>(states, nrhs, x, p, r, n, n, s));
+    }
+    launched += batch;
+  }
+  return cudaSuccess;
+}
+
+template <typename T>
 cudaError_t device_norm2(const void* vec, size_t n, double* partial, double* scratch_dev, double* host, cudaStream_t s) {
   CK(norm2_partial<T>(vec, n, partial, s));
   CK(final_sum(partial, reduce_blocks(n), 1, scratch_dev, s));
@@ -142,6 +210,8 @@ template struct Op<double>;
 template struct Op<float>;
 template cudaError_t cg_normal<double>(const Op<double>&, const void*, void*, const CgVectors&, double, int, int, CgState*, cudaStream_t);
 template cudaError_t cg_normal<float>(const Op<float>&, const void*, void*, const CgVectors&, double, int, int, CgState*, cudaStream_t);
+template cudaError_t cg_normal_multi<double>(const Op<double>&, int, const void*, void*, void*, void*, void*, double*, CgState*, int*, double, int, int, CgState*, cudaStream_t);
+template cudaError_t cg_normal_multi<float>(const Op<float>&, int, const void*, void*, void*, void*, void*, double*, CgState*, int*, double, int, int, CgState*, cudaStream_t);
 template cudaError_t device_norm2<double>(const void*, size_t, double*, double*, double*, cudaStream_t);
 template cudaError_t device_norm2<float>(const void*, size_t, double*, double*, double*, cudaStream_t);
 

@@ -21,6 +21,11 @@ struct Op {
                     const int* skip, cudaStream_t s) const;
   // full operator on nrhs spinor fields stored back to back (in[n], out[n] one full field apart), EPI_STORE
   cudaError_t apply_multi(const void* in, void* out, int nrhs, bool dagger, cudaStream_t s) const;
+  // the same with a fused epilogue per right-hand side (pipeline kernel only: check multi_fused_ok() first):
+  // partial[n * ntiles + tile], alpha of column n at alpha[n * alpha_stride], r an array like in / out
+  cudaError_t apply_multi_epi(const void* in, void* out, int nrhs, bool dagger, int epi, void* r, const double* alpha,
+                              int alpha_stride, double* partial, const int* skip, cudaStream_t s) const;
+  bool multi_fused_ok() const;
   cudaError_t hop_xpay(const void* in, const void* self, void* out, double k, int parity, cudaStream_t s) const;
 };
 
@@ -36,6 +41,15 @@ struct CgVectors {
 template <typename T>
 cudaError_t cg_normal(const Op<T>& M, const void* bprime, void* x, const CgVectors& v, double tol, int maxiter,
                       int check_every, CgState* host_state, cudaStream_t s);
+
+// nrhs independent solves M^+ M x_n = bprime_n in lock step (full operator, pipeline kernel): every stencil pass takes
+// all columns (links and clover blocks shared, lqcd_dw_apply_multi), scalars and convergence flags per column on the
+// device.  r, p, t, x, bprime: nrhs fields back to back.  states: nrhs CgState on the device, host_states: nrhs on the
+// host (final states).  partial: >= nrhs * ntiles doubles; flags: 2 ints on the device (all-done flag, ticket counter).
+template <typename T>
+cudaError_t cg_normal_multi(const Op<T>& M, int nrhs, const void* bprime, void* x, void* r, void* p, void* t, double* partial,
+                            CgState* states, int* flags, double tol, int maxiter, int check_every, CgState* host_states,
+                            cudaStream_t s);
 
 template <typename T>
 cudaError_t device_norm2(const void* vec, size_t n, double* partial, double* scratch_dev, double* host, cudaStream_t s);

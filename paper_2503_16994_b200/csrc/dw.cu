@@ -795,7 +795,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
       // epilogue (same three variants as dw_kernel)
       const size_t ooff = field_offset(g, 12, p, tile, 0, j) + (size_t)(rhs * a.rhs_stride);
       if (a.epi == EPI_AXPY_NORM) {
-        const T al = (T)(*a.alpha);
+        const T al = (T)a.alpha[(size_t)rhs * a.alpha_stride];
         T2<T>* rq = a.r + ooff;
 #pragma unroll
         for (int c = 0; c < 12; c++) {
@@ -1418,6 +1418,10 @@ int dw_num_partials(const Geom& g, int recon, int diag, int parity) {
   if (!c.use) c = pipe_half_config<T>(g, recon, diag, parity);
   return c.use ? g.ntiles : direct_config<T>(g, recon, diag, parity).grid;   // pipeline: one partial sum per tile
 }
+template <typename T>
+bool dw_uses_pipe(const Geom& g, int recon, int diag, int parity) { return pipe_config<T>(g, recon, diag, parity).use; }
+template bool dw_uses_pipe<double>(const Geom&, int, int, int);
+template bool dw_uses_pipe<float>(const Geom&, int, int, int);
 template int dw_num_partials<double>(const Geom&, int, int, int);
 template int dw_num_partials<float>(const Geom&, int, int, int);
 

@@ -29,12 +29,18 @@ struct DwArgs {
   unsigned int* sched;                 // pipeline kernel: {next tile, finished CTAs} of its tile scheduler (NULL: static)
   int nrhs;                            // > 1: in / out are arrays of nrhs spinor fields rhs_stride complex numbers apart
   long long rhs_stride;                //      (several right-hand sides share the links and the clover term)
+  int alpha_stride;                    //      in doubles: right-hand side n takes its alpha from alpha[n * alpha_stride] (0: one alpha for all)
   int nsplit;                          //      pipeline kernel: a tile's right-hand sides are shared out over nsplit work units (set by launch_pipe)
 };
 
 // number of per-CTA partial sums an EPI_*_NORM launch with these arguments writes to DwArgs::partial
 template <typename T>
 int dw_num_partials(const Geom& g, int recon, int diag, int parity);
+
+// does launch_dw run these arguments on the pipeline kernel (dw_pipe_kernel)?  Only then may nrhs > 1 be combined with
+// a reducing epilogue (partial[n * ntiles + tile], alpha[n * alpha_stride])
+template <typename T>
+bool dw_uses_pipe(const Geom& g, int recon, int diag, int parity);
 
 // one-line description of the kernel launch_dw would use (lqcd_dw_plan); dw_set_mode: lqcd_set_option("dw_mode")
 template <typename T>

@@ -64,6 +64,12 @@ cudaError_t final_sum(const double* partial, int n, int nvals, double* result, c
 cudaError_t cg_init_state(CgState* st, const double* partial, int n, double tol, cudaStream_t s);
 cudaError_t cg_reduce_alpha(CgState* st, const double* partial, int n, cudaStream_t s);
 cudaError_t cg_reduce_beta(CgState* st, const double* partial, int n, cudaStream_t s);
+// the same for nrhs columns in lock step (partial sums of column c at partial + c * n; flags: {all finished, ticket})
+cudaError_t cg_init_state_multi(CgState* st, int nrhs, const double* partial, int n, double tol, int* flags, cudaStream_t s);
+cudaError_t cg_reduce_alpha_multi(CgState* st, int nrhs, const double* partial, int n, int* flags, cudaStream_t s);
+cudaError_t cg_reduce_beta_multi(CgState* st, int nrhs, const double* partial, int n, cudaStream_t s);
+template <typename T>
+cudaError_t cg_update_xp_multi(const CgState* st, int nrhs, void* x, void* p, const void* r, size_t n, size_t stride, cudaStream_t s);
 // x += alpha p ; p = r + beta p   (skips according to st->done)
 template <typename T> cudaError_t cg_update_xp(const CgState* st, void* x, void* p, const void* r, size_t ncomplex, cudaStream_t s);
 // r -= st->alpha * q, |r|^2 partials (reduce_blocks(ncomplex) of them); skipped once st->done is set
