@@ -389,7 +389,7 @@ enum { PIPE_CONS_WARPS = 8, PIPE_HALO_THREADS = 96, PIPE_THREADS = 384, PIPE_MAX
        PIPE_TQ = 4 };
 struct PipeBars {
   uint64_t full_sp[2], empty_sp[2];   // spinor tile buffer(s): one in fp64, two in fp32 (pipe_nspb)
-  uint64_t full_h[4], empty_h[4];   // two halo buffers (full lattice), three (half lattice)
+  uint64_t full_h[4], empty_h[4];   // two halo buffers (full lattice), three or four (half lattice)
   uint64_t full[PIPE_MAX_SLOTS], empty[PIPE_MAX_SLOTS];
   uint64_t tq_full[PIPE_TQ], tq_empty[PIPE_TQ];   // tile queue: the producer lane tells the other warps which tile is next
   int tq[PIPE_TQ];
@@ -857,7 +857,15 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
 // streams both parities of the links (all of them are used: forward hops take the links of the output parity, backward
 // hops those of the input parity), one parity of the input spinor, of the self spinor (DIAG_PRE) and of the blocks.
 // =====================================================================================================
-enum { HALF_NHB = 3, HALF_NF = 32, HALF_HS = HALF_NHB * HALF_NF, HALF_CLV_ROWS = 9 };
+#ifndef HALF_NHB32
+#define HALF_NHB32 4
+#endif
+enum { HALF_NF = 32, HALF_CLV_ROWS = 9 };
+// halo buffers of the half-lattice kernel (32 columns each): three in fp64 (all that fits), four in fp32 -- every halo
+// then has three stages of lead and halo rows have the stride of tile rows (D^ fp32 at 32^3 x 64 with 3 / 4 / 5 / 6
+// buffers: 0.441 / 0.422 / 0.437 / 0.434 ms)
+template <typename T> __host__ __device__ constexpr int half_nhb() { return sizeof(T) == 4 ? HALF_NHB32 : 3; }
+template <typename T> __host__ __device__ constexpr int half_hs() { return half_nhb<T>() * HALF_NF; }
 
 template <typename T, int NCU>
 __device__ __forceinline__ void halo_load_half(const Geom& g, const DwArgs<T>& a, const int* __restrict__ tab, const int mu,
@@ -870,14 +878,14 @@ __device__ __forceinline__ void halo_load_half(const Geom& g, const DwArgs<T>& a
     const int jn = face_site(mu, q, f, kind == 0 ? 0 : 3);
     if (kind < 2) {
       const T2<T>* src = a.in + field_offset(g, 12, q, kind == 0 ? tf : tb, 0, jn);
-      T2<T>* dst = hb + kind * 12 * HALF_HS + f;
+      T2<T>* dst = hb + kind * 12 * half_hs<T>() + f;
 #pragma unroll
-      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * HALF_HS, src + c * TV);
+      for (int c = 0; c < 12; c++) cp_async_elem<T>(dst + c * half_hs<T>(), src + c * TV);
     } else {
       const T2<T>* src = a.U + field_offset(g, 4 * NCU, q, tb, mu * NCU, jn);
-      T2<T>* dst = hb + 24 * HALF_HS + f;
+      T2<T>* dst = hb + 24 * half_hs<T>() + f;
 #pragma unroll
-      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * HALF_HS, src + c * TV);
+      for (int c = 0; c < NCU; c++) cp_async_elem<T>(dst + c * half_hs<T>(), src + c * TV);
     }
   }
 }
@@ -900,15 +908,15 @@ __device__ __forceinline__ void hop_one(const Geom& g, const DwArgs<T>& a, const
     if (MU == 0) jn = j - l0h + ((l[0] + 1) >> 1);
     else jn = j + stride;
     const T2<T>* ps = cr ? hb + fidx : sp_in + jn;
-    hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, cr ? (int)HALF_HS : TV, TV, sg, a.has_theta, a.theta[MU], acc);
+    hop_dir<T, RECON, MU, true, false>(ps, ub + (p * NCU) * TV + j, cr ? half_hs<T>() : TV, TV, sg, a.has_theta, a.theta[MU], acc);
   } else {
     const bool cr = (l[MU] == 0);
     int jn;
     if (MU == 0) jn = j - l0h + ((l[0] - 1) >> 1);
     else jn = j - stride;
-    const T2<T>* ps = cr ? hb + 12 * HALF_HS + fidx : sp_in + jn;
-    const T2<T>* us = cr ? hb + 24 * HALF_HS + fidx : ub + (q * NCU) * TV + jn;
-    hop_dir<T, RECON, MU, false, false>(ps, us, cr ? (int)HALF_HS : TV, cr ? (int)HALF_HS : TV, -sg, a.has_theta, a.theta[MU], acc);
+    const T2<T>* ps = cr ? hb + 12 * half_hs<T>() + fidx : sp_in + jn;
+    const T2<T>* us = cr ? hb + 24 * half_hs<T>() + fidx : ub + (q * NCU) * TV + jn;
+    hop_dir<T, RECON, MU, false, false>(ps, us, cr ? half_hs<T>() : TV, cr ? half_hs<T>() : TV, -sg, a.has_theta, a.theta[MU], acc);
   }
 }
 
@@ -931,14 +939,14 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   T2<T>* sp_base = reinterpret_cast<T2<T>*>(smem_raw);      //   [12][TV] input spinor, parity q; exchange area after the hops
                                                             //   [12][TV] self spinor, parity p (SELF)
   T2<T>* ring = sp_base + NSPB * SPW * TV;                  // nslot x [2][NCU][TV] (block stages use the first 9 rows)
-  T2<T>* halo = ring + nslot * 2 * NCU * TV;                // [24 + NCU][HALF_HS]: three halo buffers of 32 columns
-  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * HALF_HS);
+  T2<T>* halo = ring + nslot * 2 * NCU * TV;                // [24 + NCU][half_hs<T>()]: halo buffers of 32 columns
+  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * half_hs<T>());
   if (tid == 0) {
     for (int i = 0; i < NSPB; i++) {
       mbar_init(&bars->full_sp[i], 1);
       mbar_init(&bars->empty_sp[i], PIPE_CONS_WARPS);
     }
-    for (int i = 0; i < HALF_NHB; i++) {
+    for (int i = 0; i < half_nhb<T>(); i++) {
       mbar_init(&bars->full_h[i], PIPE_HALO_THREADS);
       mbar_init(&bars->empty_h[i], PIPE_CONS_WARPS);
     }
@@ -1016,7 +1024,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           mbar_wait_relaxed(&bars->empty_h[hp.slot], hp.ph ^ 1u);
           halo_load_half<T, NCU>(g, a, tab, mu, q, halo + hp.slot * HALF_NF, lt);
           cp_async_arrive_noinc(&bars->full_h[hp.slot]);
-          hp.advance(HALF_NHB);
+          hp.advance(half_nhb<T>());
         }
       }
     }
@@ -1063,7 +1071,7 @@ dw_pipe_half_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
           mbar_arrive(&bars->empty_h[b]);                                                                              \
         }                                                                                                              \
         rp.advance(nslot);                                                                                             \
-        hp.advance(HALF_NHB);                                                                                          \
+        hp.advance(half_nhb<T>());                                                                                          \
       }
       LQCD_HALF_HOP(0)
       LQCD_HALF_HOP(1)
@@ -1276,7 +1284,7 @@ static PipeCfg pipe_half_config(const Geom& g, int recon, int diag, int parity) 
   const int ncu = recon == 12 ? 6 : 9;
   const size_t sp = (size_t)pipe_nspb<T>() * (diag == DIAG_POST ? 12 : 24) * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
-  const size_t halo = (size_t)(24 + ncu) * HALF_HS * sizeof(T2<T>);
+  const size_t halo = (size_t)(24 + ncu) * half_hs<T>() * sizeof(T2<T>);
   const size_t budget = (size_t)g.smem_optin - 256;
   if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
   int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
