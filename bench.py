@@ -326,9 +326,9 @@ NCU_TRAFFIC = {
         "capture": "profiles/r02_dw_pipe_kernel_f64_full.txt",
         "plan": "dw_pipe_kernel<double,18,1> grid=148 threads=384 smem=227696 ring_slots=3 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
     ("48x48x48x96", "f32", 18): {
-        "bytes": 8046863000 + 1009083000,
+        "bytes": 8046250000 + 1008283000,
         "capture": "profiles/r02_dw_pipe_kernel_f32_full.txt",
-        "plan": "dw_pipe_kernel<float,18,1> grid=148 threads=384 smem=157040 ring_slots=4 halo_buffers=2 tile=4x4x4x4 sweep=1 chunk=3x3"},
+        "plan": "dw_pipe_kernel<float,18,1> grid=148 threads=384 smem=190832 ring_slots=4 halo_buffers=4 tile=4x4x4x4 sweep=1 chunk=3x3"},
 }
 
 

@@ -113,6 +113,9 @@ __device__ __forceinline__ void hop_dir(const T2<T>* __restrict__ psi, const T2<
   }
 }
 
+#ifndef PIPE_NHB32
+#define PIPE_NHB32 4
+#endif
 #ifndef PIPE_NSPB32
 #define PIPE_NSPB32 2
 #endif
@@ -373,12 +376,17 @@ struct CloverStage<T, C0, 0> {
 
 // The pipeline kernel is written for 4x4x4x4 tiles: TV = 128 sites of one parity, every face 2*TV/4 = 64 columns.
 // With both fixed at compile time every shared-memory access of the arithmetic warps is an immediate offset from
-// one base register, and the two halo buffers interleave into rows of 2*PIPE_NF = PIPE_TV columns, i.e. halo rows
+// one base register, and a pair of halo buffers interleaves into rows of 2*PIPE_NF = PIPE_TV columns, i.e. halo rows
 // have the same stride as tile rows and a hop needs no stride select.
 // Spinor-tile buffers of the pipeline kernels.  With one buffer the next tile's spinor can only be requested once the
 // arithmetic warps are done with the hops of this one, and its trip from DRAM is covered by the clover stages alone;
 // fp32 has the shared memory for a second buffer (fp64 does not), and the request then goes out a whole tile ahead.
 template <typename T> __host__ __device__ constexpr int pipe_nspb() { return sizeof(T) == 4 ? PIPE_NSPB32 : 1; }
+// Halo buffers of the full-lattice kernel: pairs of them interleave into rows of PIPE_TV columns (so halo rows have the
+// stride of tile rows), one pair in fp64 (all that fits), two pairs in fp32: a halo can then be gathered a whole tile
+// ahead (profile: 11 % of the arithmetic warps' samples were waits for the halos of the third and fourth hop; Dw fp32 at
+// 48^3 x 96 with 2 / 3 / 4 buffers: 1.562 / 1.512 / 1.502 ms).
+template <typename T> __host__ __device__ constexpr int pipe_nhb() { return sizeof(T) == 4 ? PIPE_NHB32 : 2; }
 // Clover stages placed between the two pairs of hop stages (the rest follows the last hop).  fp32: half of them, so that
 // every halo has three stages of lead.  fp64, with its single spinor buffer: one -- the spinor tile is released after
 // the last hop, and the more stages follow it the more time the next tile's spinor has to arrive from DRAM; the halos,
@@ -554,7 +562,7 @@ __device__ __forceinline__ void halo_load(const Geom& g, const DwArgs<T>& a, con
 template <typename T, int RECON, int DIAG>
 __global__ void __launch_bounds__(PIPE_THREADS, 1)
 dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
-  constexpr int nhb = 2;   // halo buffers: columns [0, PIPE_NF) and [PIPE_NF, PIPE_TV) of the halo rows
+  constexpr int nhb = pipe_nhb<T>();   // halo buffers: columns [0, PIPE_NF) and [PIPE_NF, PIPE_TV) of the rows of a pair
   constexpr int NCU = (RECON == 12) ? 6 : 9;
   constexpr int NSTC = (DIAG == DIAG_PRE) ? 36 / NCU : 0;   // clover stages per tile
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -568,7 +576,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
   T2<T>* sp0 = reinterpret_cast<T2<T>*>(smem_raw);  // NSPB x [2][12][TV] spinor tile
   T2<T>* ring = sp0 + NSPB * 24 * TV;               // nslot x [2][NCU][TV]
   T2<T>* halo = ring + nslot * 2 * NCU * TV;        // [24 + NCU][PIPE_TV]: both halo buffers
-  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + (24 + NCU) * TV);
+  PipeBars* bars = reinterpret_cast<PipeBars*>(halo + ((nhb + 1) / 2) * (24 + NCU) * TV);
   if (tid == 0) {
     for (int i = 0; i < NSPB; i++) {
       mbar_init(&bars->full_sp[i], 1);
@@ -681,7 +689,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         const T2<T>* in_r = a.in + rhs * a.rhs_stride;
         for (int mu = 0; mu < 4; mu++) {
           mbar_wait_relaxed(&bars->empty_h[hp.slot], hp.ph ^ 1u);
-          halo_load<T, NCU>(g, a, in_r, tab, mu, halo + hp.slot * PIPE_NF, lt);
+          halo_load<T, NCU>(g, a, in_r, tab, mu, halo + (hp.slot >> 1) * (24 + NCU) * TV + (hp.slot & 1) * PIPE_NF, lt);
           cp_async_arrive_noinc(&bars->full_h[hp.slot]);
           hp.advance(nhb);
         }
@@ -722,7 +730,7 @@ dw_pipe_kernel(const Geom g, const DwArgs<T> a, const int nslot) {
         mbar_wait(&bars->full_h[b], hp.ph);                                                                      \
         mbar_wait(&bars->full[rp.slot], rp.ph);                                                                  \
         if (live)                                                                                                \
-          hop_pair<T, RECON, MU>(g, a, sp, ring + rp.slot * 2 * NCU * TV, halo + b * PIPE_NF, p, j, l, x3,     \
+          hop_pair<T, RECON, MU>(g, a, sp, ring + rp.slot * 2 * NCU * TV, halo + (b >> 1) * (24 + NCU) * TV + (b & 1) * PIPE_NF, p, j, l, x3, \
                                  nonper, sg, acc);                                                               \
         __syncwarp();                                                                                            \
         if (lane == 0) {                                                                                         \
@@ -1257,7 +1265,7 @@ static PipeCfg pipe_config(const Geom& g, int recon, int diag, int parity) {
   const int ncu = recon == 12 ? 6 : 9;
   const size_t sp = (size_t)pipe_nspb<T>() * 24 * g.TV * sizeof(T2<T>);
   const size_t slot = (size_t)2 * ncu * g.TV * sizeof(T2<T>);
-  const size_t halo = (size_t)(24 + ncu) * PIPE_TV * sizeof(T2<T>);   // both buffers
+  const size_t halo = (size_t)((pipe_nhb<T>() + 1) / 2) * (24 + ncu) * PIPE_TV * sizeof(T2<T>);   // pairs of buffers
   const size_t budget = (size_t)g.smem_optin - 256;   // 256 B: the kernel's static shared memory
   if (budget < sp + halo + sizeof(PipeBars) + 2 * slot) return c;
   int nslot = (int)((budget - sp - halo - sizeof(PipeBars)) / slot);
@@ -1402,13 +1410,13 @@ void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int 
   const char* tn = sizeof(T) == 8 ? "double" : "float";
   const PipeCfg hc = pipe_half_config<T>(g, recon, diag, parity);
   if (hc.use) {
-    snprintf(buf, (size_t)len, "dw_pipe_half_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=3 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
-             tn, recon, diag, hc.grid, (int)PIPE_THREADS, hc.smem, hc.nslot, g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
+    snprintf(buf, (size_t)len, "dw_pipe_half_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=%d tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
+             tn, recon, diag, hc.grid, (int)PIPE_THREADS, hc.smem, hc.nslot, half_nhb<T>(), g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
     return;
   }
   if (pc.use) {
-    snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=2 tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
-             tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
+    snprintf(buf, (size_t)len, "dw_pipe_kernel<%s,%d,%d> grid=%d threads=%d smem=%zu ring_slots=%d halo_buffers=%d tile=%dx%dx%dx%d sweep=%d chunk=%dx%d",
+             tn, recon, diag, pc.grid, (int)PIPE_THREADS, pc.smem, pc.nslot, pipe_nhb<T>(), g.b[0], g.b[1], g.b[2], g.b[3], g.sw, g.c1, g.c2);
     return;
   }
   const DirectCfg dc = direct_config<T>(g, recon, diag, parity);
