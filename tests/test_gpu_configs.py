@@ -1,4 +1,4 @@
-"""-m gpu parity at the STATED size of BASELINE.json's configs 2, 3 and 5b (SURVEY.md 8(d) protocols 2, 3, 5; config 1
+"""-m gpu parity at the STATED size of BASELINE.json's configs 2, 3, 4 and 5b (SURVEY.md 8(d) protocols 2-5; config 1
 is tests/test_gpu_dw.py::test_config1_4to4_haar_fp64, config 4's 4^3 x 8 sub-run tests/test_gpu_cg.py and
 tests/test_gpu_dw.py, config 5a tests/test_gpu_fullsize.py).
 
@@ -7,6 +7,8 @@ tests/test_gpu_dw.py, config 5a tests/test_gpu_fullsize.py).
   config 3  24^3 x 48 open, kappa = 0.1365, csw = 1.9: point-source columns solved on the GPU,
             pin P9 through two applications of the ORACLE operator per column (normal-equation residual <= 2 tol);
             the full oracle CG on the 8^3 x 16 open sub-run with the same kappa / csw, plain and even-odd + mixed.
+  config 4  32^3 x 64 Schroedinger functional, theta = 0.5, kappa = 0.1355, csw = 1.8: the even-odd operator D^ and D^+
+            against the full-size oracle on every even interior site, fp64 and fp32.
   config 5b 64^3 x 128 periodic, kappa = 0.137, csw = 1.9: D and D^+ through the kernel bench.py times, on 4096 seeded
             random sites plus the 16 lattice corners against oracle.dw_at_sites.  The oracle reads only the 3^4
             neighbourhood of a site, so only those entries of the device fields are downloaded into (lazily
@@ -242,3 +244,45 @@ def test_config5b_64x64x64x128_sampled():
             assert err.max() <= TOL[prec], (prec, dagger, err.max())
             del Uo
     B.geom_destroy(g)
+
+
+# ---------------------------------------------------------------------------------------------------- config 4
+def test_config4_32x32x32x64_sf_dhat_full_oracle():
+    """configs[3] at its stated size: the even-odd operator D^ and D^+ (both passes of the half-lattice pipeline kernel,
+    full grid of 148 CTAs, 8192 tiles) on the 32^3 x 64 Schroedinger-functional lattice with theta = 0.5, element-wise
+    against the oracle's D^ on every even interior site, fp64 and fp32 (R14: the oracle gets the rounded fields)."""
+    L, kappa, csw = (32, 32, 32, 64), 0.1355, 1.8
+    bc, theta, phiT = B.BC_SF_ORBI, (0.5, 0.5, 0.5, 0.0), synth.SF_PHIT
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12e9:
+        pytest.skip("needs 12 GB of free device memory")
+    dev = torch.device("cuda", torch.cuda.current_device())
+    U = synth.apply_sf_boundary(L, synth.smooth_gauge_torch(L, synth.seed_for(4, 0), dev).cpu().numpy())
+    psi = synth.gaussian_spinor_torch(L, synth.seed_for(4, 1), dev).cpu().numpy()
+    A = oracle.clover_blocks(L, U, kappa, csw, bc=bc, phiT=phiT)
+    Ai = oracle.clover_inverse(L, A)
+    x = np.arange(synth.vol(L))
+    par = np.zeros_like(x)
+    for mu in range(4):
+        par += x % L[mu]
+        x = x // L[mu]
+    even = (par % 2 == 0) & interior(L, bc)
+    lat = Lattice(L, bc, theta, synth.SF_PHI0, phiT)
+    lat.set_gauge(U, precs=(B.F64, B.F32))
+    lat.build_clover(kappa, csw, precs=(B.F64, B.F32), inverse=True)
+    assert B.geom_info(lat.g)[0] == [4, 4, 4, 4]
+    for prec in (B.F64, B.F32):
+        assert "dw_pipe_half_kernel" in B.dw_plan(lat.g, prec, B.RECON_18, True, parity=0)
+        # the library's own blocks against the oracle's first (fp64), then the operator on the oracle's rounding of them
+        Uo, psio, Ao, Aio = (round_f32(U), round_f32(psi), round_f32(A), round_f32(Ai)) if prec == B.F32 else (U, psi, A, Ai)
+        src = lat.spinor(psi, prec)
+        tmp = lat.alloc(B.FIELD_SPINOR, prec)
+        for dagger in (False, True):
+            ref = oracle.dhat(L, Uo, psio, kappa, Ao, Aio, bc=bc, theta=theta, dagger=dagger)
+            dst = lat.alloc(B.FIELD_SPINOR, prec)
+            dst.zero_()
+            B.dw_eo_apply(lat.g, kappa, lat.U[(prec, 18)], lat.A[prec], lat.Ainv[prec], src, dst, tmp, dagger, prec, 18)
+            got = lat.spinor_to_host(dst, prec)
+            assert site_rel_err(got, ref, even) <= TOL[prec] * 2, (prec, dagger)
+            del dst
+    lat.close()
