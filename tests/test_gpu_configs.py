@@ -127,6 +127,38 @@ def test_config3_24x24x24x48_open_p9():
     lat.close()
 
 
+def test_config3_24x24x24x48_open_lock_step_p9():
+    """The same at the stated size for the lock-step solver (lqcd_cg_solve_multi): three of the point-source columns in
+    one call; P9 through two applications of the ORACLE operator per column, and the iteration count and solution of one
+    column against the column-by-column solver (same arithmetic per column)."""
+    L, kappa, csw, tol = (24, 24, 24, 48), 0.1365, 1.9, 1e-10
+    U, A, lat = _open_setup(L, kappa, csw, synth.seed_for(3, 0), dev_gen=True)
+    y, bc = (0, 0, 0, L[3] // 2), B.BC_OPEN
+    cols = (0, 7, 11)
+    srcs = [synth.point_source(L, y, c // 3, c % 3) for c in cols]
+    fb = B.field_bytes(lat.g, B.FIELD_SPINOR)
+    b = torch.empty(len(cols) * fb, dtype=torch.uint8, device="cuda")
+    for n, src in enumerate(srcs):
+        b[n * fb:(n + 1) * fb].copy_(lat.spinor(src))
+    x = torch.empty_like(b)
+    ws = torch.empty(B.cg_multi_workspace_bytes(lat.g, len(cols)), dtype=torch.uint8, device="cuda")
+    infos = B.cg_solve_multi(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], b, x, len(cols), ws, tol=tol, maxiter=10000)
+    frozen = ~interior(L, bc)
+    for n, src in enumerate(srcs):
+        got = lat.spinor_to_host(x[n * fb:(n + 1) * fb])
+        bp = oracle.dw(L, U, src, kappa, A, bc=bc, dagger=True)
+        r = src - oracle.dw(L, U, got, kappa, A, bc=bc)
+        rn = np.linalg.norm(oracle.dw(L, U, r, kappa, A, bc=bc, dagger=True)) / np.linalg.norm(bp)
+        assert infos[n]["status"] == B.OK and rn <= 2 * tol, (n, rn)
+        assert abs(infos[n]["rel_resid_true"] - np.linalg.norm(r)) <= 0.5 * np.linalg.norm(r) + 1e-13
+        assert np.all(got[frozen] == 0)
+    x1, i1 = _solve(lat, kappa, srcs[1], tol, eo_mixed=False)
+    got1 = lat.spinor_to_host(x[fb:2 * fb])
+    assert i1["iters"] == infos[1]["iters"]
+    assert np.linalg.norm(got1 - x1) <= 1e-10 * np.linalg.norm(x1)
+    lat.close()
+
+
 def synth_parity(L):
     n = np.arange(synth.vol(L))
     p = np.zeros_like(n)
