@@ -609,6 +609,7 @@ struct SolveCtx {
   double* partial;
   double* scratch;     // 8 doubles on the device
   CgState* state;
+  unsigned int* sched = nullptr;   // SCHED_POOL_PAIRS zeroed counter pairs (CgVectors::sched_pool)
 };
 
 template <typename T>
@@ -635,7 +636,7 @@ lqcd_status solve_normal(const SolveCtx& c, const void* bp, void* x, int* iters,
   Op<double> M = make_op<double>(c, c.v64[3]);
   const size_t n = M.ncomplex();
   CgVectors v;
-  v.r = c.v64[0]; v.p = c.v64[1]; v.t = c.v64[2]; v.partial = c.partial; v.state = c.state;
+  v.r = c.v64[0]; v.p = c.v64[1]; v.t = c.v64[2]; v.partial = c.partial; v.state = c.state; v.sched_pool = c.sched;
   CgState hs;
   const int check = c.parm->check_every > 0 ? c.parm->check_every : 16;
   *outer = 0;
@@ -650,7 +651,7 @@ lqcd_status solve_normal(const SolveCtx& c, const void* bp, void* x, int* iters,
   // mixed precision: r = bp - M^+M x (fp64); e = CG32(r) to inner_tol; x += e
   Op<float> M32 = make_op<float>(c, c.v32[4]);
   CgVectors w;
-  w.r = c.v32[1]; w.p = c.v32[2]; w.t = c.v32[3]; w.partial = c.partial; w.state = c.state;
+  w.r = c.v32[1]; w.p = c.v32[2]; w.t = c.v32[3]; w.partial = c.partial; w.state = c.state; w.sched_pool = c.sched;
   void* r64 = c.v64[0];
   void* t64 = c.v64[1];
   void* q64 = c.v64[2];
@@ -719,6 +720,8 @@ lqcd_status lqcd_cg_solve(const lqcd_geom* h, const lqcd_dirac* d, const lqcd_cg
   c.partial = (double*)ws.take(partial_len(g) * sizeof(double));
   c.scratch = (double*)ws.take(64);
   c.state = (CgState*)ws.take(sizeof(CgState));
+  c.sched = (unsigned int*)ws.take((size_t)SCHED_POOL_PAIRS * 2 * sizeof(unsigned int));
+  CKS(cudaMemsetAsync(c.sched, 0, (size_t)SCHED_POOL_PAIRS * 2 * sizeof(unsigned int), as_stream(stream)), "memset");
   const size_t nfull = spinor_complex(g);
   cudaStream_t s = c.s;
   lqcd_status st = LQCD_OK;

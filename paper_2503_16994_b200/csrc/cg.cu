@@ -162,6 +162,11 @@ cudaError_t cg_normal(const Op<T>& M, const void* bprime, void* x, const CgVecto
   static const bool want_graph = [] { const char* e = getenv("LQCD_CG_GRAPH"); return !(e && e[0] == '0'); }();
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t gs = s, own = nullptr;
+  // the captured launches keep their tile-scheduler counters for every replay: give them this solve's own
+  struct PoolGuard {
+    explicit PoolGuard(unsigned int* p) { if (p) dw_set_sched_pool(p, SCHED_POOL_PAIRS); }
+    ~PoolGuard() { dw_set_sched_pool(nullptr, 0); }
+  } pool_guard(v.sched_pool);
   if (want_graph && maxiter >= check_every) {
     if (s == nullptr) { CK(cudaStreamCreate(&own)); gs = own; }
     cudaGraph_t graph = nullptr;

@@ -35,7 +35,9 @@ struct CgVectors {
   void* t;
   double* partial;   // >= max(ntiles, 2*reduce_blocks) doubles
   CgState* state;    // device
+  unsigned int* sched_pool = nullptr;   // device, zeroed: SCHED_POOL_PAIRS pairs of tile-scheduler counters of this solve
 };
+enum { SCHED_POOL_PAIRS = 128 };
 
 // Solve M^+ M x = bprime from x = 0 (bprime = M^+ b already formed).  Leaves the final state in *host_state.
 template <typename T>

@@ -1310,7 +1310,15 @@ static PipeCfg pipe_half_config(const Geom& g, int recon, int diag, int parity) 
   return c;
 }
 
+static thread_local unsigned int* t_sched_base = nullptr;
+static thread_local int t_sched_pairs = 0, t_sched_next = 0;
+void dw_set_sched_pool(unsigned int* base, int npairs) {
+  t_sched_base = npairs > 0 ? base : nullptr;
+  t_sched_pairs = npairs;
+  t_sched_next = 0;
+}
 static unsigned int* sched_slot(const Geom& g) {
+  if (t_sched_base != nullptr && g.sched != nullptr && pipe_dynamic()) return t_sched_base + 2 * (t_sched_next++ % t_sched_pairs);
   static std::atomic<unsigned> launch_no(0);
   // one pair of scheduler counters per launch in flight (a pool of SCHED_SLOTS pairs owned by the geometry, handed out
   // round-robin): launches of the same geometry running concurrently on different streams do not share a counter

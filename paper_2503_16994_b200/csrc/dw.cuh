@@ -47,6 +47,11 @@ template <typename T>
 void dw_describe(const Geom& g, int recon, int diag, int parity, char* buf, int len);
 bool dw_set_mode(const char* name);
 bool dw_set_pipe_grid(int n);
+// Tile-scheduler counters for the pipeline-kernel launches of the CALLING THREAD: while set (base != NULL), launches
+// take their {next tile, finished CTAs} pair from these npairs zeroed pairs (round robin) instead of the geometry's
+// pool.  A solver that replays its launches as a CUDA graph sets this to counters of its own (in its workspace), so
+// that two solves on one geometry running on different streams can never share a counter.
+void dw_set_sched_pool(unsigned int* base, int npairs);
 
 template <typename T>
 cudaError_t launch_dw(const Geom& g, const DwArgs<T>& a, int recon, int diag, cudaStream_t s);

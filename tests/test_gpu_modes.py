@@ -458,3 +458,46 @@ def test_full_grid_launches_repeat_bit_for_bit(prec):
     if prec == B.F64:   # (fp32 blocks with an inverse come from the one-thread-per-site kernel: equal up to one rounding)
         assert torch.equal(A2, A) and torch.equal(Ai2, Ai)
     lat.close()
+
+
+def test_concurrent_solves_on_one_geometry():
+    """Two lqcd_cg_solve calls on ONE geometry from two host threads on two CUDA streams, ten times: iteration counts
+    and solutions must be those of the serial solves, bit for bit.  (Each solve replays its iterations as a CUDA graph
+    whose stencil launches keep their tile-scheduler counters; they come from the solve's own workspace, not from the
+    geometry's pool, so that two solves can never share one.)"""
+    import threading
+    L, kappa, csw = (16, 16, 16, 16), 0.13, 1.5
+    dev = torch.device("cuda", torch.cuda.current_device())
+    lat = Lattice(L)
+    lat.set_gauge(synth.smooth_gauge_torch(L, 701, dev))
+    lat.build_clover(kappa, csw)
+    srcs = [lat.spinor(synth.gaussian_spinor_torch(L, 702 + i, dev)) for i in range(2)]
+    ws = [lat.alloc(B.FIELD_WORKSPACE) for _ in range(2)]
+    ref = []
+    for i in range(2):
+        x = lat.alloc(B.FIELD_SPINOR)
+        info = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], srcs[i], x, ws[i], tol=1e-8, maxiter=2000)
+        ref.append((x.clone(), info["iters"]))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for rep in range(10):
+        outs = [lat.alloc(B.FIELD_SPINOR) for _ in range(2)]
+        infos, errs = [None, None], []
+
+        def work(i):
+            try:
+                infos[i] = B.cg_solve(lat.g, kappa, lat.U[(B.F64, 18)], lat.A[B.F64], srcs[i], outs[i], ws[i], tol=1e-8,
+                                      maxiter=2000, stream=streams[i])
+            except Exception as e:   # surfaces in the main thread below
+                errs.append(e)
+
+        torch.cuda.synchronize()
+        threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        torch.cuda.synchronize()
+        assert not errs, errs
+        for i in range(2):
+            assert infos[i]["iters"] == ref[i][1] and torch.equal(outs[i], ref[i][0]), (rep, i)
+    lat.close()
